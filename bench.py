@@ -1,0 +1,399 @@
+#!/usr/bin/env python
+"""bench.py -- times the hot path of the B200 HiCR copy engine and prints ONE JSON line.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config NAME] [--impl reference]
+
+A *step* is one pass of the whole hot path over one batch of synthetic input:
+``hicr_memcpy_batch`` (descriptor ingest + validation, binning, copy kernels, counter
+accumulation) followed by ``hicr_fence``.  The default workload is BASELINE.json's
+config 2 ("bulk aligned": 2 slots x 1 GiB, 65,536 descriptors of 4 KiB per step, four
+pairwise-disjoint descriptor sets rotated so a page is re-touched only after 2 GiB of
+other traffic).  ``metric`` = effective GB/s = (bytes read + bytes written) / time.
+
+  value        device-resident descriptor tables, inputs in HBM when timing starts
+  e2e          the same call with HOST descriptor tables (the step's input) copied to
+               the device inside the timed region and the fence's counter read-back
+  roofline     dominant copy kernel, CUDA events recorded by the library around it
+  cpu_baseline the CPU oracle (oracle/, as it stands) on the host cores, same workload
+
+N > 1 (torchrun): the path shards by slot ownership with no data-path collective -- every
+rank owns its own slots and descriptor sets (seed + rank); weak scaling; the time is the
+max over ranks.  ``--impl reference`` times the oracle instead (rank 0 only).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import workloads as W  # noqa: E402
+
+METRIC = "memory-slot memcpy effective GB/s (read+write)"
+UNIT = "GB/s"
+
+
+# --------------------------------------------------------------------------- workloads
+def make_workload(name: str, rank: int = 0):
+    seed = W.BASE_SEED + 1000 * rank
+    if name == "bulk":
+        return W.bulk_aligned(seed=seed)
+    if name == "bulk_small":            # CPU-sized stand-in used by the tests of this file
+        return W.bulk_aligned(n_desc=1024, slot_bytes=32 * W.MiB, n_sets=4, seed=seed)
+    if name == "tiny":
+        return W.tiny(seed=seed)
+    if name == "heavy_a":
+        return W.heavy_tailed("a", seed=seed)
+    if name == "heavy_b":
+        return W.heavy_tailed("b", seed=seed)
+    if name == "chain":
+        return W.chained_epochs(seed=seed)
+    raise SystemExit("unknown --config %s" % name)
+
+
+WORKLOAD_TEXT = {
+    "bulk": "config 2 bulk aligned: 2 slots x 1 GiB, 65536 x 4 KiB descriptors per step, 4 KiB-aligned, "
+            "random page permutation, 1 fence per step",
+    "bulk_small": "config 2 scaled down (test only)",
+    "tiny": "config 1 tiny: 2 slots x 1 MiB, 256 descriptors of 1..4096 B, 1 fence per step",
+    "heavy_a": "config 3a heavy-tailed: 64 slots x 256 MiB, 100000 descriptors, power law 1.3 on 16 B..16 MiB",
+    "heavy_b": "config 3b heavy-tailed: 64 slots x 256 MiB, log-uniform 16 B..16 MiB until full",
+    "chain": "config 4 chained epochs: 1 slot x 256 MiB, 64 epochs x 65536 descriptors of 8..256 B",
+}
+
+
+def shard_report(per_rank_bytes, per_rank_descs, elapsed_ms_max, steps):
+    """Whole-job aggregate over ranks (weak scaling, no data-path collective): all ranks'
+    units over the slowest rank's time."""
+    secs = elapsed_ms_max / 1e3
+    return {
+        "value": float(sum(per_rank_bytes)) / secs / 1e9,
+        "descs_per_s": float(sum(per_rank_descs)) / secs,
+        "ms_per_step": elapsed_ms_max / steps,
+    }
+
+
+# --------------------------------------------------------------------------- clocks
+class ClockSampler:
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    REASONS = {
+        0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+        0x80: "hw_power_brake", 0x2: "applications_clocks", 0x100: "display_clock", 0x10: "sync_boost",
+    }
+
+    def __init__(self, index: int, period_s: float = 0.005):
+        self.samples, self.reasons, self.period = [], 0, period_s
+        self._stop = threading.Event()
+        self._thr = None
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self._nv = pynvml
+            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self._nv = None
+
+    def _run(self):
+        nv = self._nv
+        while not self._stop.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
+                self.reasons |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
+            except Exception:
+                try:
+                    self.reasons |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
+                except Exception:
+                    pass
+            self._stop.wait(self.period)
+
+    def start(self):
+        if self._nv:
+            self._thr = threading.Thread(target=self._run, daemon=True)
+            self._thr.start()
+
+    def stop(self):
+        if self._thr:
+            self._stop.set()
+            self._thr.join()
+        names = sorted(n for bit, n in self.REASONS.items() if self.reasons & bit)
+        return {
+            "sm_mhz": float(np.median(self.samples)) if self.samples else None,
+            "sm_max_mhz": self.max_mhz,
+            "reasons": names,
+            "samples": len(self.samples),
+        }
+
+
+# --------------------------------------------------------------------------- CPU oracle arm
+def host_cores() -> int:
+    try:
+        return len(os.sched_getaffinity(0))
+    except Exception:
+        return os.cpu_count() or 1
+
+
+def oracle_steps(w, n_steps: int, warmup: int = 0, budget_s: float = None, total_budget_s: float = None):
+    """Run the CPU oracle (single-threaded byte loops, as it stands) over the workload's
+    descriptor sets, one fence per step.  With ``total_budget_s`` every step is a bounded
+    sample: the first ``m`` descriptors of its set, ``m`` chosen from one calibration step so
+    that warmup + n_steps steps fit the budget.  Returns (seconds per step, bytes moved per
+    step (read + written), descriptors per step)."""
+    from oracle import Oracle
+    imgs = [w.slot_image(s) for s in range(len(w.slot_sizes))]
+    o = Oracle()
+    for i in imgs:
+        o.slot_register(i)
+    frac = 1.0
+    if total_budget_s is not None:
+        t0 = time.perf_counter()
+        assert o.memcpy_batch(w.epochs[0])[0] == 0 and o.fence() == 0
+        t_full = time.perf_counter() - t0
+        frac = min(1.0, total_budget_s / (t_full * (warmup + n_steps)))
+    sets = [np.ascontiguousarray(e[: max(1, int(round(len(e) * frac)))]) for e in w.epochs]
+    times, moved, units = [], [], []
+    t_begin = time.perf_counter()
+    for k in range(warmup + n_steps):
+        e = sets[k % len(sets)]
+        t0 = time.perf_counter()
+        rc, _ = o.memcpy_batch(e)
+        assert rc == 0
+        assert o.fence() == 0
+        dt = time.perf_counter() - t0
+        if k >= warmup:
+            times.append(dt)
+            moved.append(2.0 * float(e["size"].sum()))
+            units.append(len(e))
+        if budget_s is not None and k >= warmup and time.perf_counter() - t_begin > budget_s:
+            break
+    return times, moved, units
+
+
+def bytes_per_step(w) -> float:
+    return 2.0 * w.bytes_copied / len(w.epochs)
+
+
+def descs_per_step(w) -> float:
+    return w.n_descs / len(w.epochs)
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    w = make_workload(args.config)
+    times, moved, units = oracle_steps(w, args.steps, warmup=args.warmup, total_budget_s=args.reference_seconds)
+    total = float(sum(times))
+    gbs = sum(moved) / total / 1e9
+    full = descs_per_step(w)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": len(times), "warmup": args.warmup, "ms_per_step": 1e3 * total / len(times),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": WORKLOAD_TEXT[args.config], "name": args.config},
+        "descs_per_s": sum(units) / total,
+        "cpu_baseline": {"value": gbs, "unit": UNIT, "cores": 1, "kind": "oracle",
+                         "sample": "%d steps, each the first %d of the %d descriptors of its set; "
+                                   "host cores available: %d" % (len(times), units[0], full, host_cores())},
+        "e2e": {"value": gbs, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# --------------------------------------------------------------------------- CUDA arm
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def run_cuda(args):
+    import torch
+    import paper_2509_01425_b200 as hicr
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback "
+                         "(use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    w = make_workload(args.config, rank)
+    stream = torch.cuda.Stream()
+    K, Wm = args.steps, max(3, args.warmup)
+    n_sets = len(w.epochs)
+    with torch.cuda.stream(stream):
+        ctx = hicr.Context(local, stream.cuda_stream)
+        bufs = [torch.from_numpy(w.slot_image(s)).to("cuda", non_blocking=False) for s in range(len(w.slot_sizes))]
+        ids = [ctx.slot_register(b) for b in bufs]
+        host_tables = [np.ascontiguousarray(e) for e in w.epochs]
+        dev_tables = [torch.from_numpy(t.view(np.uint8).copy()).cuda() for t in host_tables]
+        n_per = [len(t) for t in host_tables]
+        stream.synchronize()
+
+        def step_device(i):
+            ctx.memcpy_batch(dev_tables[i % n_sets], n=n_per[i % n_sets])
+            ctx.fence()
+
+        def step_host(i):
+            ctx.memcpy_batch(host_tables[i % n_sets])
+            ctx.fence()
+
+        # ---- device-resident arm (value + roofline)
+        ctx.profile_enable(True)
+        for i in range(Wm):
+            step_device(i)
+        prof = np.zeros(4)
+        n_prof = 0
+        clocks = ClockSampler(local)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        l0 = ctx.launch_count()
+        clocks.start()
+        t_host0 = time.perf_counter()
+        e0.record(stream)
+        for i in range(K):
+            step_device(i)
+            if i % 8 == 0:                      # sampled read of the library's per-kernel events
+                prof += np.asarray(ctx.profile_read())
+                n_prof += 1
+        e1.record(stream)
+        barrier()
+        t_host = time.perf_counter() - t_host0
+        clk = clocks.stop()
+        launches = ctx.launch_count() - l0
+        ms = e0.elapsed_time(e1)
+        ctx.profile_enable(False)
+
+        # ---- fence cost alone: an epoch with one 1-descriptor batch
+        one = dev_tables[0]
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            ctx.memcpy_batch(one, n=1)
+            ctx.fence()
+        torch.cuda.synchronize()
+        tf = time.perf_counter()
+        for _ in range(50):
+            ctx.memcpy_batch(one, n=1)
+            ctx.fence()
+        fence_us = (time.perf_counter() - tf) / 50 * 1e6
+
+        # ---- end-to-end arm: host descriptor tables in, counters out, every step
+        for i in range(Wm):
+            step_host(i)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        g0.record(stream)
+        for i in range(K):
+            step_host(i)
+        g1.record(stream)
+        barrier()
+        ms_e2e = g0.elapsed_time(g1)
+        counters = [ctx.slot_counters(s) for s in ids]
+
+    def allmax(x):
+        if dist is None:
+            return x
+        t = torch.tensor([x], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        return float(t.item())
+
+    ms_max, ms_e2e_max = allmax(ms), allmax(ms_e2e)
+    bps, dps = bytes_per_step(w), descs_per_step(w)
+    agg = shard_report([bps * K] * world, [dps * K] * world, ms_max, K)
+    agg_e2e = shard_report([bps * K] * world, [dps * K] * world, ms_e2e_max, K)
+
+    if rank == 0:
+        peak, peak_src = load_peaks()
+        prof /= max(1, n_prof)
+        kernel_ms = {"plan": prof[0], "copy_warp": prof[1], "copy_cta": prof[2], "all": prof[3]}
+        dom = "copy_warp" if prof[1] >= prof[2] else "copy_cta"
+        achieved = bps / (kernel_ms[dom] * 1e-3) / 1e9 if kernel_ms[dom] > 0 else 0.0
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        if os.path.exists(tp):
+            try:
+                traffic = json.load(open(tp)).get(args.config, {}).get("dram_bytes_per_launch")
+            except Exception:
+                traffic = None
+        # CPU oracle beside it, same workload, bounded to about 10 s of CPU work
+        cpu = None
+        if not args.no_cpu_baseline:
+            times, moved, _ = oracle_steps(make_workload(args.config, 0), 10 ** 6, warmup=1, budget_s=args.cpu_seconds)
+            cpu_gbs = sum(moved) / float(sum(times)) / 1e9
+            cpu = {"value": cpu_gbs, "unit": UNIT, "cores": 1, "kind": "oracle",
+                   "sample": "%d full steps of the same workload in %.1f s (host cores available: %d)"
+                             % (len(times), sum(times), host_cores())}
+        line = {
+            "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
+            "ms_per_step": agg["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "u8", "data": "synthetic",
+            "config": {"workload": WORKLOAD_TEXT[args.config], "name": args.config,
+                       "descriptor_tables": "device-resident", "l2": "inputs larger than L2: %d MiB touched per step, "
+                       "%d rotating disjoint sets" % (bps / 2 ** 20, n_sets), "sharding": "independent slots per rank"},
+            "descs_per_s": agg["descs_per_s"], "fence_us": fence_us, "host_ms_per_step": 1e3 * t_host / K,
+            "frac_of_hbm_peak": agg["value"] / world / peak,
+            "e2e": {"value": agg_e2e["value"], "unit": UNIT,
+                    "h2d_bytes_per_step": int(32 * dps), "d2h_bytes_per_step": int(64 + 16 * len(ids)),
+                    "ms_per_step": agg_e2e["ms_per_step"], "what": "host descriptor tables in, slot counters out"},
+            "gpu_launches": int(launches),
+            "kernel_ms": kernel_ms,
+            "roofline": {"bound": "hbm", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak, "unit": UNIT,
+                         "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         "algorithmic_bytes_per_launch": bps},
+            "cpu_baseline": cpu,
+            "clocks": clk,
+            "counters_ok": bool(sum(c[0] for c in counters) == sum(c[1] for c in counters)),
+        }
+        print(json.dumps(line))
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2000)
+    ap.add_argument("--warmup", type=int, default=20)
+    ap.add_argument("--config", default="bulk", choices=sorted(WORKLOAD_TEXT))
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU work of the cpu_baseline leg")
+    ap.add_argument("--reference-seconds", type=float, default=90.0,
+                    help="--impl reference: CPU work of the whole run (each step a bounded sample)")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_cuda(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -1,0 +1,219 @@
+/*
+ * hicr.h -- C ABI of the B200-native HiCR memory-slot copy engine and token channels.
+ *
+ * What this library is: the data-parallel hot path of the HiCR runtime-support-layer
+ * model (arxiv 2509.01425, cited below as PAPER.md:<line>), i.e. the Communication
+ * Manager's `memcpy` between registered Local Memory Slots, completed by `fence`
+ * (listing PAPER.md:524-535), plus the Channels frontend's
+ * fixed-size-token circular buffer.  One GPU, one memory space
+ * (that GPU's HBM).  Every step of the path runs in hand-written sm_100a CUDA kernels;
+ * there is no CPU fallback: without a CUDA device every call returns HICR_ERR_CUDA.
+ *
+ * Conventions
+ *   - C linkage, `int` status return (HICR_OK = 0, errors negative), no exceptions and
+ *     no callbacks cross the boundary.
+ *   - All sizes and offsets are bytes, uint64_t (SURVEY.md S8(c) reading 2).
+ *   - "device pointer" = an address in the memory of the device given to hicr_init;
+ *     "host pointer" = ordinary host memory.  Each argument says which it is.
+ *   - The library never owns slot storage (it "will record the provided
+ *     information"); the caller keeps it alive until hicr_slot_unregister/hicr_finalize.
+ *   - All device work is enqueued on the cudaStream_t given to hicr_init.
+ *   - A context and its channels are driven by one host thread at a time.
+ */
+#ifndef HICR_H
+#define HICR_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes -------------------------------------------------------------- */
+#define HICR_OK                     0
+#define HICR_ERR_INVALID_ARG      (-1)  /* NULL where a pointer is required, capacity 0, ... */
+#define HICR_ERR_INVALID_SLOT     (-2)  /* slot id not registered (or unregistered twice)    */
+#define HICR_ERR_OUT_OF_BOUNDS    (-3)  /* off > slot size or size > slot size - off         */
+#define HICR_ERR_UNSUPPORTED_SPACE (-4) /* pointer is not memory of this device: "Otherwise,
+                                           it will be rejected"               */
+#define HICR_ERR_NO_CAPACITY      (-5)  /* slot table / work queue / allocation exhausted    */
+#define HICR_ERR_CUDA             (-6)  /* a CUDA runtime call failed; hicr_last_cuda_error  */
+#define HICR_ERR_BUSY             (-7)  /* object still referenced (e.g. slot used by a channel) */
+
+typedef struct hicr_ctx hicr_ctx_t;          /* opaque context  */
+typedef struct hicr_channel hicr_channel_t;  /* opaque SPSC channel */
+typedef struct hicr_mpsc hicr_mpsc_t;        /* opaque non-locking MPSC channel set */
+typedef uint32_t hicr_slot_t;                /* dense slot id, valid for one context */
+
+#define HICR_MAX_SLOTS 4096u
+
+/* One transfer.  Field order follows the paper's call
+ *   cmm->memcpy(dst, 0, message, 0, messageSize)
+ * i.e. destination slot, destination offset, source slot, source offset, size.
+ * 32 bytes, little endian, no padding. */
+typedef struct hicr_desc {
+    uint32_t dst_slot;
+    uint32_t src_slot;
+    uint64_t dst_off;
+    uint64_t src_off;
+    uint64_t size;
+} hicr_desc_t;
+
+/* ---- context (plumbing) ----------------------------------------------------------- */
+
+/* Create a context on CUDA device `device`; all work goes to `cuda_stream` (a
+ * cudaStream_t passed as void*; NULL = the legacy default stream).  *out receives the
+ * context.  The context owns the device-side slot table, work queues, control blocks
+ * and staging buffers.  Errors: HICR_ERR_INVALID_ARG, HICR_ERR_CUDA (no device). */
+int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream);
+
+/* Wait for outstanding work, free everything the context owns (never slot storage). */
+int hicr_finalize(hicr_ctx_t *ctx);
+
+/* Static text for a status code. */
+const char *hicr_strerror(int status);
+
+/* Text of the last CUDA runtime error seen by this context ("" if none). Host pointer,
+ * owned by the context. */
+const char *hicr_last_cuda_error(hicr_ctx_t *ctx);
+
+/* ---- memory slots ------------------------------------------- */
+
+/* Register an existing device allocation [dev_ptr, dev_ptr + size) as a Local Memory
+ * Slot: "manual registration of an existing memory allocation as a new local memory
+ * slot by specifying its address, size".  Any base alignment; size 0 is
+ * allowed (then dev_ptr may be NULL).  Sent/received counters start at 0.  *out
+ * receives a dense id.  Errors: HICR_ERR_UNSUPPORTED_SPACE if dev_ptr is not device
+ * memory of this context's device; HICR_ERR_NO_CAPACITY beyond HICR_MAX_SLOTS live
+ * and retired ids. */
+int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_t *out);
+
+/* Forget a slot (storage untouched).  The caller must have fenced every transfer that
+ * names it.  HICR_ERR_INVALID_SLOT on unknown id or double unregister; HICR_ERR_BUSY
+ * while a live channel uses it as its ring. */
+int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot);
+
+/* Per-slot message counters (host pointers out): `sent` = transfers/tokens whose source
+ * was this slot, `recv` = those whose destination was this slot; cumulative since
+ * registration (SURVEY.md S8(c) readings 7, 8: the "expected number of incoming and
+ * outgoing data transfers" of PAPER.md:375, one message per descriptor / per token).
+ * Values are defined immediately after hicr_fence or after a completed channel call. */
+int hicr_slot_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64_t *recv);
+
+/* ---- memcpy + fence (listing PAPER.md:532-534) ------------------- */
+
+/* Initiate `n` transfers dst[dst_off + i] = src[src_off + i], i < size.
+ *
+ *   descs            array of n hicr_desc_t.  descs_on_device == 0: host pointer; it is
+ *                    validated and consumed before return (the caller may free it).
+ *                    descs_on_device != 0: device pointer; it must stay alive and
+ *                    unchanged until the next hicr_fence; it is validated on the device.
+ *   first_bad        host pointer or NULL; on a host-side validation error receives the
+ *                    lowest invalid index.
+ *
+ * Asynchronous: "The completion of a memory transfer is not guaranteed after the
+ * function call returns"; completion and visibility only at hicr_fence.
+ * All-or-nothing (reading 10): if any descriptor names an unregistered slot
+ * (HICR_ERR_INVALID_SLOT) or a range outside its slot (HICR_ERR_OUT_OF_BOUNDS) the
+ * whole batch has no effect and counts nothing; the status is that of the lowest bad
+ * index (destination checked before source).  Host-resident tables report it here;
+ * device-resident tables report it at hicr_fence.  A zero-size transfer moves nothing
+ * and still counts one message (reading 4).  n == 0 is a no-op.
+ *
+ * Caller contract inside one epoch (= between two fences; reading 5): destination
+ * ranges are pairwise disjoint and no destination range overlaps any source range.
+ * Sources may overlap; src and dst may be the same slot.  Violations are undefined. */
+int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint64_t n, int descs_on_device,
+                      uint64_t *first_bad);
+
+/* Block the host until every transfer initiated since the previous fence is complete
+ * and visible to the host and to later device work; publish the slot counters; close
+ * the epoch ("suspend execution until the expected number of incoming and outgoing data
+ * transfers have been completed"; bare fence() as in PAPER.md:534).
+ * Returns the first deferred error of the epoch (device-validated batches) or HICR_OK;
+ * with nothing outstanding it returns at once.  Batches of the epoch other than the
+ * failed one are unaffected. */
+int hicr_fence(hicr_ctx_t *ctx);
+
+/* After hicr_fence returned a deferred error: which batch of that epoch (0-based) and
+ * which descriptor index in it was the first bad one.  Host pointers out (may be NULL). */
+int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad);
+
+/* ---- channels -------------------------------------------------- */
+
+/* SPSC channel over the ring slot: `capacity` tokens of `token_bytes` bytes each; the
+ * slot must hold capacity * token_bytes bytes (the pre-allocated circular buffer of
+ * PAPER.md:642).  head = tokens ever pushed, tail = tokens ever popped, both 64-bit
+ * counters in device memory, 0 at creation.  capacity >= 1, token_bytes >= 1. */
+int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes, uint64_t capacity,
+                        hicr_channel_t **out);
+int hicr_channel_destroy(hicr_channel_t *ch);
+
+/* (head, tail) as of the last completed call on this channel.  Host pointers out. */
+int hicr_channel_counters(hicr_channel_t *ch, uint64_t *head, uint64_t *tail);
+
+/* Push min(n_tokens, capacity - (head - tail)) tokens, in order, from slot `src` at
+ * byte offset src_off: token j goes to ring position (head + j) mod capacity; head is
+ * advanced after the payload is visible ("the producer knows where to push the next
+ * message, as long as the buffer has not filled up").  *n_pushed (host
+ * pointer) receives the count; 0 with n_tokens > 0 = full.  The source range of
+ * n_tokens * token_bytes bytes must lie inside `src`.  Complete on return.  Counts one
+ * message per token: sent(src), recv(ring).  The k decision is taken on the device from
+ * the device-resident counters. */
+int hicr_channel_push(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, uint64_t n_tokens,
+                      uint64_t *n_pushed);
+
+/* Pop k = min(max_tokens, head - tail) tokens in FIFO order into slot `dst` at dst_off:
+ * token j comes from ring position (tail + j) mod capacity; tail is advanced once per
+ * call after the reads are done ("the consumer notifies that a message has been
+ * consumed").  *n_popped receives k; 0 = empty.  The range of
+ * k * token_bytes bytes must lie inside `dst` (else HICR_ERR_OUT_OF_BOUNDS, no effect).
+ * Complete on return.  Counts sent(ring), recv(dst). */
+int hicr_channel_pop(hicr_channel_t *ch, hicr_slot_t dst, uint64_t dst_off, uint64_t max_tokens,
+                     uint64_t *n_popped);
+
+/* Device-resident SPSC run: one kernel in which a producer CTA performs, for
+ * i < n_batches, a blocking push of batch_tokens[i] tokens (waiting on the device for
+ * room) from `src` (consecutive tokens starting at src_off) while a consumer CTA
+ * concurrently pops whatever is available into `dst` (consecutive from dst_off) until
+ * all sum(batch_tokens) tokens are through.  batch_tokens: host pointer, consumed
+ * before return.  Blocks until done.  On return head and tail have advanced by the sum
+ * and the counters by one message per token, exactly as the equivalent sequence of
+ * hicr_channel_push / hicr_channel_pop calls would leave them.  Requires an empty ring
+ * (head == tail) at entry. */
+int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, hicr_slot_t dst,
+                        uint64_t dst_off, const uint64_t *batch_tokens, uint64_t n_batches);
+
+/* Non-locking MPSC ("dedicated buffers per producer"): `producers` SPSC
+ * rings, rings[p] the ring slot of producer p (host pointer to `producers` ids). */
+int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rings, uint64_t token_bytes,
+                     uint64_t capacity, hicr_mpsc_t **out);
+int hicr_mpsc_destroy(hicr_mpsc_t *m);
+int hicr_mpsc_counters(hicr_mpsc_t *m, uint32_t producer, uint64_t *head, uint64_t *tail);
+
+/* Device-resident MPSC run: one producer CTA per producer (one per SM on B200 when
+ * producers = 148) pushes tokens_per_producer tokens from src_slots[p] (offset 0) into
+ * its own ring in batches of at most max_batch tokens, waiting for room on the device;
+ * a single consumer CTA polls the rings round-robin and pops what is available into
+ * dst_slots[p] (offset 0).  Per-producer FIFO.  src_slots / dst_slots: host pointers to
+ * `producers` ids.  Blocks until done; counters as for hicr_channel_stream. */
+int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_slot_t *dst_slots,
+                     uint64_t tokens_per_producer, uint64_t max_batch);
+
+/* ---- measurement hooks (plumbing) -------------------------------------------------- */
+
+/* Kernel launches issued by this context since hicr_init (host pointer out). */
+int hicr_launch_count(hicr_ctx_t *ctx, uint64_t *launches);
+
+/* With profiling on, every hicr_memcpy_batch records CUDA events around its kernels on
+ * the context's stream.  hicr_profile_read (after a fence) returns, for the LAST batch,
+ * the device time in milliseconds of: [0] the plan/binning kernel, [1] the warp-per-
+ * descriptor copy kernel, [2] the CTA-per-chunk copy kernel, [3] all three end to end.
+ * ms: host pointer to 4 floats. */
+int hicr_profile_enable(hicr_ctx_t *ctx, int on);
+int hicr_profile_read(hicr_ctx_t *ctx, float *ms);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HICR_H */

@@ -1,0 +1,558 @@
+// hicr_channel.cu -- fixed-size-token channels on device counters (a8, a9, a10).
+//
+// "Channels operate by exchanging pre-allocated circular buffers ... By pre-allocating
+// the buffers, the producer knows where to push the next message, as long as the buffer
+// has not filled up. At that point the producer may not send any more messages until the
+// consumer notifies that a message has been consumed.".  MPSC non-locking:
+// "dedicated buffers per producer".
+//
+// head (tokens ever pushed) and tail (tokens ever popped) are 64-bit counters in device
+// memory; the push/pop decision k is taken on the device from them.  Payload first, then
+// the counter with release semantics; the other side reads the counter with acquire.
+//
+//   channel_push_kernel / channel_pop_kernel  one call = one launch; the grid splits the
+//        (at most two) contiguous spans into pieces; the last CTA to finish publishes the
+//        counter, the slot message counts and the call result (mapped pinned memory).
+//   spsc_stream_kernel   cooperative launch, CTA 0 = producer, CTA 1 = consumer, the whole
+//        push/pop sequence in one kernel (no host round trip per call).
+//   mpsc_stream_kernel   cooperative launch, CTA p < P = producer p (one per SM for P = 148),
+//        CTA P = the single consumer; its warps each poll and drain their own rings.
+#include "hicr_internal.cuh"
+
+#include <algorithm>
+#include <cstring>
+
+struct hicr_channel {
+    hicr_ctx *ctx = nullptr;
+    hicr_slot_t ring = 0;
+    uint64_t T = 0, C = 0;
+    hicr::ChannelState *d_state = nullptr;
+    unsigned int *d_ticket = nullptr;
+    uint64_t head = 0, tail = 0;   // host mirror as of the last completed call
+};
+
+struct hicr_mpsc {
+    hicr_ctx *ctx = nullptr;
+    uint32_t P = 0;
+    uint64_t T = 0, C = 0;
+    std::vector<hicr_slot_t> rings;
+    hicr::ChannelState *d_state = nullptr;   // [P]
+    uint64_t *d_ptrs = nullptr;              // [3 * P]: ring base, source base, sink base
+    std::vector<uint64_t> head, tail;
+};
+
+namespace hicr {
+
+constexpr int kCallThreads = 256;
+constexpr uint64_t kPieceBytes = 16384;     // per-CTA piece of a host-call push/pop
+constexpr int kStreamThreads = 512;   // SPSC stream: 2 CTAs on 2 SMs
+constexpr int kMpscThreads = 256;     // MPSC stream: P + 1 CTAs must be co-resident, 2 per SM at <= 128 registers
+
+// Copy `len` logical bytes starting at logical ring byte `rb` (wraps at ring_bytes).
+template <int U, bool TO_RING>
+__device__ __forceinline__ void ring_copy(unsigned char *ring, uint64_t ring_bytes, uint64_t rb,
+                                          unsigned char *lin, uint64_t len, int gtid, int gsize)
+{
+    const uint64_t first = min(len, ring_bytes - rb);
+    if (TO_RING) {
+        copy_span<U, kLdL2>(ring + rb, lin, first, gtid, gsize);
+        if (len > first) copy_span<U, kLdL2>(ring, lin + first, len - first, gtid, gsize);
+    } else {
+        copy_span<U, kLdL2>(lin, ring + rb, first, gtid, gsize);
+        if (len > first) copy_span<U, kLdL2>(lin + first, ring, len - first, gtid, gsize);
+    }
+}
+
+// (a8) push / (a9) pop as one launch.  `lin` = the linear side (source slot for push,
+// destination slot for pop) already offset; lin_room = bytes available there.
+template <bool PUSH>
+__global__ void __launch_bounds__(kCallThreads)
+channel_call_kernel(ChannelState *st, unsigned int *ticket, unsigned char *ring, uint64_t T, uint64_t C,
+                    unsigned char *lin, uint64_t lin_room, uint64_t n, unsigned long long *cnt_lin_out,
+                    unsigned long long *cnt_ring_out, CallResult *res)
+{
+    const unsigned long long head = st->head, tail = st->tail;
+    uint64_t k;
+    long long status = HICR_OK;
+    if (PUSH) k = min((unsigned long long)n, (unsigned long long)C - (head - tail));
+    else {
+        k = min((unsigned long long)n, head - tail);
+        if (k * T > lin_room) {   // destination range of the k tokens must fit (no effect otherwise)
+            status = HICR_ERR_OUT_OF_BOUNDS;
+            k = 0;
+        }
+    }
+    const uint64_t bytes = k * T, ring_bytes = C * T;
+    const uint64_t rb0 = ((PUSH ? head : tail) % C) * T;
+    for (uint64_t off = (uint64_t)blockIdx.x * kPieceBytes; off < bytes; off += (uint64_t)gridDim.x * kPieceBytes) {
+        const uint64_t len = min(kPieceBytes, bytes - off);
+        ring_copy<4, PUSH>(ring, ring_bytes, (rb0 + off) % ring_bytes, lin + off, len, threadIdx.x, kCallThreads);
+    }
+    __threadfence();
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    if (atomicAdd(ticket, 1u) != gridDim.x - 1) return;
+    // last CTA: every CTA has read head/tail and finished its pieces
+    __threadfence();
+    *ticket = 0;
+    if (PUSH) {
+        st_release(&st->head, head + k);
+        *cnt_lin_out += k;     // sent(src)
+        *cnt_ring_out += k;    // recv(ring)
+        res->head = head + k;
+        res->tail = tail;
+    } else {
+        st_release(&st->tail, tail + k);
+        *cnt_ring_out += k;    // sent(ring)
+        *cnt_lin_out += k;     // recv(dst)
+        res->head = head;
+        res->tail = tail + k;
+    }
+    res->k = k;
+    res->status = status;
+    __threadfence_system();
+}
+
+__device__ __forceinline__ void backoff(unsigned &ns)
+{
+    __nanosleep(ns);
+    if (ns < 256) ns *= 2;
+}
+
+// Device-resident SPSC run.  CTA 0 produces, CTA 1 consumes; co-residency is guaranteed by
+// the cooperative launch.  cnt[0..3] = &sent[src], &recv[ring], &sent[ring], &recv[dst].
+__global__ void __launch_bounds__(kStreamThreads)
+spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C, unsigned char *src,
+                   unsigned char *dst, const uint64_t *__restrict__ batches, uint64_t n_batches, uint64_t total,
+                   unsigned long long *c_sent_src, unsigned long long *c_recv_ring,
+                   unsigned long long *c_sent_ring, unsigned long long *c_recv_dst, CallResult *res)
+{
+    __shared__ unsigned long long sh_k;
+    const uint64_t ring_bytes = C * T;
+    const int tid = threadIdx.x;
+    if (blockIdx.x == 0) {
+        unsigned long long head = st->head;
+        uint64_t pushed = 0;
+        for (uint64_t b = 0; b < n_batches; b++) {
+            uint64_t rem = batches[b];
+            while (rem) {            // blocking push: wait for room, push what fits
+                if (tid == 0) {
+                    unsigned ns = 20;
+                    unsigned long long room;
+                    while ((room = C - (head - ld_acquire(&st->tail))) == 0) backoff(ns);
+                    sh_k = min((unsigned long long)rem, room);
+                }
+                __syncthreads();
+                const uint64_t k = sh_k;
+                ring_copy<8, true>(ring, ring_bytes, (head % C) * T, src + pushed * T, k * T, tid, kStreamThreads);
+                __syncthreads();     // every thread's payload stores are issued
+                if (tid == 0) {
+                    __threadfence();
+                    st_release(&st->head, head + k);
+                }
+                head += k;
+                pushed += k;
+                rem -= k;
+            }
+        }
+    } else {
+        unsigned long long tail = st->tail;
+        uint64_t popped = 0;
+        while (popped < total) {
+            if (tid == 0) {
+                unsigned ns = 20;
+                unsigned long long avail;
+                while ((avail = ld_acquire(&st->head) - tail) == 0) backoff(ns);
+                sh_k = avail;
+            }
+            __syncthreads();
+            const uint64_t k = sh_k;
+            ring_copy<8, false>(ring, ring_bytes, (tail % C) * T, dst + popped * T, k * T, tid, kStreamThreads);
+            __syncthreads();         // every thread's ring loads have returned (their stores were issued)
+            if (tid == 0) {
+                __threadfence();
+                st_release(&st->tail, tail + k);
+            }
+            tail += k;
+            popped += k;
+        }
+        if (tid == 0) {
+            atomicAdd(c_sent_src, total);
+            atomicAdd(c_recv_ring, total);
+            atomicAdd(c_sent_ring, total);
+            atomicAdd(c_recv_dst, total);
+            res->k = total;
+            res->head = ld_acquire(&st->head);
+            res->tail = tail;
+            res->status = HICR_OK;
+            __threadfence_system();
+        }
+    }
+}
+
+// Device-resident non-locking MPSC run.  ptrs = [ring base | source base | sink base] x P.
+// slot_ids = [ring | source | sink] x P for the message counters.
+__global__ void __launch_bounds__(kMpscThreads, 2)
+mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const uint64_t *__restrict__ ptrs,
+                   const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch,
+                   unsigned long long *sent, unsigned long long *recv)
+{
+    const uint64_t ring_bytes = C * T;
+    const int tid = threadIdx.x;
+    if (blockIdx.x < P) {
+        // ---- producer p: blocking pushes of at most max_batch tokens
+        __shared__ unsigned long long sh_k;
+        const uint32_t p = blockIdx.x;
+        ChannelState *s = st + p;
+        unsigned char *ring = reinterpret_cast<unsigned char *>(ptrs[p]);
+        unsigned char *src = reinterpret_cast<unsigned char *>(ptrs[P + p]);
+        unsigned long long head = s->head;
+        uint64_t pushed = 0;
+        while (pushed < tokens) {
+            if (tid == 0) {
+                unsigned ns = 20;
+                unsigned long long room;
+                while ((room = C - (head - ld_acquire(&s->tail))) == 0) backoff(ns);
+                sh_k = min(min((unsigned long long)(tokens - pushed), (unsigned long long)max_batch), room);
+            }
+            __syncthreads();
+            const uint64_t k = sh_k;
+            ring_copy<2, true>(ring, ring_bytes, (head % C) * T, src + pushed * T, k * T, tid, kMpscThreads);
+            __syncthreads();
+            if (tid == 0) {
+                __threadfence();
+                st_release(&s->head, head + k);
+            }
+            head += k;
+            pushed += k;
+        }
+        return;
+    }
+    // ---- the single consumer: warp w polls and drains rings w, w + nwarps, ...
+    const int lane = tid & 31, warp = tid >> 5, nwarps = kMpscThreads / 32;
+    bool all_done = false;
+    unsigned ns = 20;
+    while (!all_done) {
+        all_done = true;
+        bool progressed = false;
+        for (uint32_t p = warp; p < P; p += nwarps) {
+            ChannelState *s = st + p;
+            unsigned long long tail = 0, head = 0;
+            if (lane == 0) {
+                tail = __ldcg(&s->tail);   // only this warp ever writes it (read at L2, where the release store went)
+                head = tail < tokens ? ld_acquire(&s->head) : tail;
+            }
+            tail = __shfl_sync(0xffffffffu, tail, 0);
+            head = __shfl_sync(0xffffffffu, head, 0);
+            if (tail >= tokens) continue;
+            all_done = false;
+            const uint64_t k = head - tail;
+            if (k == 0) continue;
+            progressed = true;
+            unsigned char *ring = reinterpret_cast<unsigned char *>(ptrs[p]);
+            unsigned char *dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]);
+            ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
+            __syncwarp();
+            if (lane == 0) {
+                __threadfence();
+                st_release(&s->tail, tail + k);
+                if (tail + k == tokens) {   // this ring is through: one message per token (reading 15)
+                    atomicAdd(&sent[slot_ids[P + p]], (unsigned long long)tokens);
+                    atomicAdd(&recv[slot_ids[p]], (unsigned long long)tokens);
+                    atomicAdd(&sent[slot_ids[p]], (unsigned long long)tokens);
+                    atomicAdd(&recv[slot_ids[2 * P + p]], (unsigned long long)tokens);
+                }
+            }
+        }
+        if (!progressed && !all_done) backoff(ns); else ns = 20;
+    }
+}
+
+// The kernel wrote the result into mapped pinned memory before the stream synchronize returned.
+static CallResult read_result(hicr_ctx *ctx)
+{
+    const volatile CallResult *v = ctx->h_call;
+    CallResult r;
+    r.k = v->k;
+    r.head = v->head;
+    r.tail = v->tail;
+    r.status = v->status;
+    return r;
+}
+
+static int slot_ok(hicr_ctx *ctx, hicr_slot_t s)
+{
+    return s < ctx->slots.size() && ctx->slots[s].size != kInvalidSize;
+}
+
+}  // namespace hicr
+
+using namespace hicr;
+
+extern "C" {
+
+int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes, uint64_t capacity,
+                        hicr_channel_t **out)
+{
+    if (!ctx || !out) return HICR_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;   // capacity >= 1
+    if (!slot_ok(ctx, ring)) return HICR_ERR_INVALID_SLOT;
+    if (capacity > ~0ull / token_bytes || capacity * token_bytes > ctx->slots[ring].size)
+        return HICR_ERR_OUT_OF_BOUNDS;
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    hicr_channel *ch = new hicr_channel();
+    ch->ctx = ctx;
+    ch->ring = ring;
+    ch->T = token_bytes;
+    ch->C = capacity;
+    cudaError_t e = cudaMalloc(&ch->d_state, sizeof(ChannelState) + 128);
+    if (e == cudaSuccess) e = cudaMemsetAsync(ch->d_state, 0, sizeof(ChannelState) + 128, ctx->stream);
+    if (e != cudaSuccess) {
+        cudaFree(ch->d_state);
+        delete ch;
+        return cuda_fail(ctx, e, "hicr_channel_create");
+    }
+    ch->d_ticket = reinterpret_cast<unsigned int *>(ch->d_state + 1);
+    ctx->ring_refs[ring]++;
+    *out = ch;
+    return HICR_OK;
+}
+
+int hicr_channel_destroy(hicr_channel_t *ch)
+{
+    if (!ch) return HICR_ERR_INVALID_ARG;
+    (void)cudaStreamSynchronize(ch->ctx->stream);
+    cudaFree(ch->d_state);
+    ch->ctx->ring_refs[ch->ring]--;
+    delete ch;
+    return HICR_OK;
+}
+
+int hicr_channel_counters(hicr_channel_t *ch, uint64_t *head, uint64_t *tail)
+{
+    if (!ch || !head || !tail) return HICR_ERR_INVALID_ARG;
+    *head = ch->head;
+    *tail = ch->tail;
+    return HICR_OK;
+}
+
+static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uint64_t off, uint64_t n,
+                        uint64_t *n_out)
+{
+    if (!ch || !n_out) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = ch->ctx;
+    *n_out = 0;
+    if (!slot_ok(ctx, lin_slot)) return HICR_ERR_INVALID_SLOT;
+    const SlotRow &ls = ctx->slots[lin_slot];
+    if (off > ls.size) return HICR_ERR_OUT_OF_BOUNDS;
+    if (push) {
+        if (n > ~0ull / ch->T || n * ch->T > ls.size - off) return HICR_ERR_OUT_OF_BOUNDS;
+    }
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    const uint64_t max_tokens = std::min<uint64_t>(n, ch->C);
+    const uint64_t max_bytes = max_tokens * ch->T;
+    unsigned grid = (unsigned)std::min<uint64_t>(std::max<uint64_t>(1, (max_bytes + kPieceBytes - 1) / kPieceBytes),
+                                                 (uint64_t)ctx->num_sms * 4);
+    unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+    unsigned char *lin = reinterpret_cast<unsigned char *>(ls.base + off);
+    CallResult *res = ctx->d_call;
+    if (push)
+        channel_call_kernel<true><<<grid, kCallThreads, 0, ctx->stream>>>(
+            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_sent + lin_slot,
+            ctx->d_recv + ch->ring, res);
+    else
+        channel_call_kernel<false><<<grid, kCallThreads, 0, ctx->stream>>>(
+            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_recv + lin_slot,
+            ctx->d_sent + ch->ring, res);
+    ctx->launches++;
+    HICR_CUDA(ctx, cudaGetLastError());
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // "Complete on return"
+    const CallResult r = read_result(ctx);
+    ch->head = r.head;
+    ch->tail = r.tail;
+    if (r.status != HICR_OK) return (int)r.status;
+    *n_out = r.k;
+    if (push) {
+        ctx->sent[lin_slot] += r.k;
+        ctx->recv[ch->ring] += r.k;
+    } else {
+        ctx->sent[ch->ring] += r.k;
+        ctx->recv[lin_slot] += r.k;
+    }
+    return HICR_OK;
+}
+
+int hicr_channel_push(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, uint64_t n_tokens, uint64_t *n_pushed)
+{
+    return channel_call(ch, true, src, src_off, n_tokens, n_pushed);
+}
+
+int hicr_channel_pop(hicr_channel_t *ch, hicr_slot_t dst, uint64_t dst_off, uint64_t max_tokens, uint64_t *n_popped)
+{
+    return channel_call(ch, false, dst, dst_off, max_tokens, n_popped);
+}
+
+int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, hicr_slot_t dst, uint64_t dst_off,
+                        const uint64_t *batch_tokens, uint64_t n_batches)
+{
+    if (!ch || (!batch_tokens && n_batches)) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = ch->ctx;
+    if (!slot_ok(ctx, src) || !slot_ok(ctx, dst)) return HICR_ERR_INVALID_SLOT;
+    if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;
+    uint64_t total = 0;
+    for (uint64_t i = 0; i < n_batches; i++) {
+        if (batch_tokens[i] > (1ull << 48)) return HICR_ERR_OUT_OF_BOUNDS;
+        total += batch_tokens[i];
+        if (total > (1ull << 48)) return HICR_ERR_OUT_OF_BOUNDS;
+    }
+    const SlotRow &ss = ctx->slots[src], &ds = ctx->slots[dst];
+    if (total > ~0ull / ch->T) return HICR_ERR_OUT_OF_BOUNDS;
+    if (src_off > ss.size || total * ch->T > ss.size - src_off) return HICR_ERR_OUT_OF_BOUNDS;
+    if (dst_off > ds.size || total * ch->T > ds.size - dst_off) return HICR_ERR_OUT_OF_BOUNDS;
+    if (total == 0) return HICR_OK;
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    uint64_t *d_batches = nullptr;
+    HICR_CUDA(ctx, cudaMalloc(&d_batches, n_batches * 8));
+    cudaError_t e = cudaMemcpyAsync(d_batches, batch_tokens, n_batches * 8, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+        ChannelState *st = ch->d_state;
+        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+        unsigned char *sp = reinterpret_cast<unsigned char *>(ss.base + src_off);
+        unsigned char *dp = reinterpret_cast<unsigned char *>(ds.base + dst_off);
+        uint64_t T = ch->T, C = ch->C;
+        const uint64_t *bp = d_batches;
+        unsigned long long *c0 = ctx->d_sent + src, *c1 = ctx->d_recv + ch->ring, *c2 = ctx->d_sent + ch->ring,
+                           *c3 = ctx->d_recv + dst;
+        CallResult *res = ctx->d_call;
+        void *args[] = {&st, &ring, &T, &C, &sp, &dp, &bp, &n_batches, &total, &c0, &c1, &c2, &c3, &res};
+        e = cudaLaunchCooperativeKernel((const void *)spsc_stream_kernel, dim3(2), dim3(kStreamThreads), args, 0,
+                                        ctx->stream);
+        ctx->launches++;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_batches);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "hicr_channel_stream");
+    const CallResult r = read_result(ctx);
+    ch->head = r.head;
+    ch->tail = r.tail;
+    ctx->sent[src] += total;
+    ctx->recv[ch->ring] += total;
+    ctx->sent[ch->ring] += total;
+    ctx->recv[dst] += total;
+    return HICR_OK;
+}
+
+int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rings, uint64_t token_bytes,
+                     uint64_t capacity, hicr_mpsc_t **out)
+{
+    if (!ctx || !out || !rings) return HICR_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (producers == 0 || token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;
+    if (capacity > ~0ull / token_bytes) return HICR_ERR_OUT_OF_BOUNDS;
+    for (uint32_t p = 0; p < producers; p++) {
+        if (!slot_ok(ctx, rings[p])) return HICR_ERR_INVALID_SLOT;
+        if (capacity * token_bytes > ctx->slots[rings[p]].size) return HICR_ERR_OUT_OF_BOUNDS;
+    }
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    hicr_mpsc *m = new hicr_mpsc();
+    m->ctx = ctx;
+    m->P = producers;
+    m->T = token_bytes;
+    m->C = capacity;
+    m->rings.assign(rings, rings + producers);
+    m->head.assign(producers, 0);
+    m->tail.assign(producers, 0);
+    cudaError_t e = cudaMalloc(&m->d_state, sizeof(ChannelState) * producers);
+    if (e == cudaSuccess) e = cudaMemsetAsync(m->d_state, 0, sizeof(ChannelState) * producers, ctx->stream);
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ptrs, (size_t)producers * (3 * 8 + 3 * 4));
+    if (e != cudaSuccess) {
+        cudaFree(m->d_state);
+        cudaFree(m->d_ptrs);
+        delete m;
+        return cuda_fail(ctx, e, "hicr_mpsc_create");
+    }
+    for (uint32_t p = 0; p < producers; p++) ctx->ring_refs[rings[p]]++;
+    *out = m;
+    return HICR_OK;
+}
+
+int hicr_mpsc_destroy(hicr_mpsc_t *m)
+{
+    if (!m) return HICR_ERR_INVALID_ARG;
+    (void)cudaStreamSynchronize(m->ctx->stream);
+    cudaFree(m->d_state);
+    cudaFree(m->d_ptrs);
+    for (auto r : m->rings) m->ctx->ring_refs[r]--;
+    delete m;
+    return HICR_OK;
+}
+
+int hicr_mpsc_counters(hicr_mpsc_t *m, uint32_t producer, uint64_t *head, uint64_t *tail)
+{
+    if (!m || !head || !tail || producer >= m->P) return HICR_ERR_INVALID_ARG;
+    *head = m->head[producer];
+    *tail = m->tail[producer];
+    return HICR_OK;
+}
+
+int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_slot_t *dst_slots,
+                     uint64_t tokens_per_producer, uint64_t max_batch)
+{
+    if (!m || !src_slots || !dst_slots || max_batch == 0) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = m->ctx;
+    const uint32_t P = m->P;
+    const uint64_t N = tokens_per_producer;
+    if (N > (1ull << 48) / m->T) return HICR_ERR_OUT_OF_BOUNDS;
+    for (uint32_t p = 0; p < P; p++) {
+        if (!slot_ok(ctx, src_slots[p]) || !slot_ok(ctx, dst_slots[p])) return HICR_ERR_INVALID_SLOT;
+        if (N * m->T > ctx->slots[src_slots[p]].size || N * m->T > ctx->slots[dst_slots[p]].size)
+            return HICR_ERR_OUT_OF_BOUNDS;
+        if (m->head[p] != m->tail[p]) return HICR_ERR_INVALID_ARG;
+    }
+    if (N == 0) return HICR_OK;
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    // co-residency of all P + 1 CTAs is what makes the spin-waits safe
+    int per_sm = 0;
+    HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, 0));
+    if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
+
+    std::vector<uint64_t> ptrs(3 * (size_t)P);
+    std::vector<uint32_t> ids(3 * (size_t)P);
+    for (uint32_t p = 0; p < P; p++) {
+        ptrs[p] = ctx->slots[m->rings[p]].base;
+        ptrs[P + p] = ctx->slots[src_slots[p]].base;
+        ptrs[2 * P + p] = ctx->slots[dst_slots[p]].base;
+        ids[p] = m->rings[p];
+        ids[P + p] = src_slots[p];
+        ids[2 * P + p] = dst_slots[p];
+    }
+    uint32_t *d_ids = reinterpret_cast<uint32_t *>(m->d_ptrs + 3 * (size_t)P);
+    HICR_CUDA(ctx, cudaMemcpyAsync(m->d_ptrs, ptrs.data(), ptrs.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+    HICR_CUDA(ctx, cudaMemcpyAsync(d_ids, ids.data(), ids.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+    // heads/tails restart from the mirror values (they are equal per ring); the kernel
+    // works with absolute token indices, so reset the device counters to 0-based per run
+    HICR_CUDA(ctx, cudaMemsetAsync(m->d_state, 0, sizeof(ChannelState) * P, ctx->stream));
+    ChannelState *st = m->d_state;
+    uint32_t Pv = P;
+    uint64_t T = m->T, C = m->C, tok = N, mb = max_batch;
+    const uint64_t *pp = m->d_ptrs;
+    const uint32_t *ip = d_ids;
+    unsigned long long *sent = ctx->d_sent, *recv = ctx->d_recv;
+    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &sent, &recv};
+    HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_stream_kernel, dim3(P + 1), dim3(kMpscThreads),
+                                               args, 0, ctx->stream));
+    ctx->launches++;
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    for (uint32_t p = 0; p < P; p++) {
+        m->head[p] += N;
+        m->tail[p] += N;
+        ctx->sent[src_slots[p]] += N;
+        ctx->recv[m->rings[p]] += N;
+        ctx->sent[m->rings[p]] += N;
+        ctx->recv[dst_slots[p]] += N;
+    }
+    return HICR_OK;
+}
+
+}  // extern "C"

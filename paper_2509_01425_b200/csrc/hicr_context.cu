@@ -1,0 +1,291 @@
+// hicr_context.cu -- context, slot table (a1) and fence (a7) of the copy engine.
+//
+// a1  hicr_slot_register : "record the provided information and return a
+//                          memory slot object"
+// a7  hicr_fence         : "suspend execution until the expected number of
+//                          incoming and outgoing data transfers have been completed"
+#include "hicr_internal.cuh"
+
+#include <cstdio>
+#include <cstring>
+
+namespace hicr {
+
+int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what)
+{
+    if (ctx) {
+        ctx->cuda_error = std::string(cudaGetErrorName(e)) + ": " + cudaGetErrorString(e) + " in " + what;
+    }
+    (void)cudaGetLastError();  // clear the sticky-less error state
+    return HICR_ERR_CUDA;
+}
+
+static int bad_to_status(unsigned id)
+{
+    switch (id) {
+    case kBadInvalidSlot: return HICR_ERR_INVALID_SLOT;
+    case kBadOutOfBounds: return HICR_ERR_OUT_OF_BOUNDS;
+    case kBadNoCapacity: return HICR_ERR_NO_CAPACITY;
+    default: return HICR_ERR_INVALID_ARG;
+    }
+}
+
+// Read back the slot counters (device -> pinned -> host mirror).  Stream must be idle or
+// the caller synchronizes afterwards; here we synchronize.
+int refresh_counters(hicr_ctx *ctx)
+{
+    const size_t n = ctx->slots.size();
+    if (n == 0) return HICR_OK;
+    unsigned char *p = ctx->h_fence + sizeof(Ctl) * kCtlRing;
+    HICR_CUDA(ctx, cudaMemcpyAsync(p, ctx->d_sent, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
+    HICR_CUDA(ctx, cudaMemcpyAsync(p + 8 * (size_t)HICR_MAX_SLOTS, ctx->d_recv, n * 8, cudaMemcpyDeviceToHost,
+                                   ctx->stream));
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    memcpy(ctx->sent.data(), p, n * 8);
+    memcpy(ctx->recv.data(), p + 8 * (size_t)HICR_MAX_SLOTS, n * 8);
+    return HICR_OK;
+}
+
+// Complete everything enqueued so far in this epoch: copy the used control blocks and
+// the counters back, wait, fold deferred errors into the epoch state, reset the control
+// blocks and recycle staging.  final_fence distinguishes hicr_fence from the internal
+// drain that happens when an epoch issues more than kCtlRing batches.
+int drain_epoch(hicr_ctx *ctx, bool final_fence)
+{
+    const uint32_t nb = ctx->batches_in_epoch;
+    const size_t n = ctx->slots.size();
+    unsigned char *p = ctx->h_fence;
+    if (nb) HICR_CUDA(ctx, cudaMemcpyAsync(p, ctx->d_ctl, sizeof(Ctl) * nb, cudaMemcpyDeviceToHost, ctx->stream));
+    unsigned char *pc = p + sizeof(Ctl) * kCtlRing;
+    if (n && final_fence) {
+        HICR_CUDA(ctx, cudaMemcpyAsync(pc, ctx->d_sent, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
+        HICR_CUDA(ctx, cudaMemcpyAsync(pc + 8 * (size_t)HICR_MAX_SLOTS, ctx->d_recv, n * 8, cudaMemcpyDeviceToHost,
+                                       ctx->stream));
+    }
+    if (nb) HICR_CUDA(ctx, cudaMemsetAsync(ctx->d_ctl, 0, sizeof(Ctl) * nb, ctx->stream));
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    const Ctl *c = reinterpret_cast<const Ctl *>(p);
+    for (uint32_t b = 0; b < nb; b++) {
+        if (c[b].bad_inv != 0 && ctx->epoch_error == HICR_OK) {
+            const unsigned long long packed = ~c[b].bad_inv;
+            ctx->epoch_error = bad_to_status((unsigned)(packed & 15));
+            ctx->epoch_error_batch = ctx->epoch_batch_base + b;
+            ctx->epoch_error_index = packed >> 4;
+        }
+    }
+    ctx->epoch_batch_base += nb;
+    ctx->batches_in_epoch = 0;
+    if (n && final_fence) {
+        memcpy(ctx->sent.data(), pc, n * 8);
+        memcpy(ctx->recv.data(), pc + 8 * (size_t)HICR_MAX_SLOTS, n * 8);
+    }
+    for (auto &b : ctx->used_stage) ctx->free_stage.push_back(b);
+    ctx->used_stage.clear();
+    return HICR_OK;
+}
+
+}  // namespace hicr
+
+using namespace hicr;
+
+extern "C" {
+
+const char *hicr_strerror(int status)
+{
+    switch (status) {
+    case HICR_OK: return "ok";
+    case HICR_ERR_INVALID_ARG: return "invalid argument";
+    case HICR_ERR_INVALID_SLOT: return "invalid memory slot";
+    case HICR_ERR_OUT_OF_BOUNDS: return "range outside its memory slot";
+    case HICR_ERR_UNSUPPORTED_SPACE: return "memory space not supported by this communication manager";
+    case HICR_ERR_NO_CAPACITY: return "capacity exhausted";
+    case HICR_ERR_CUDA: return "CUDA runtime error";
+    case HICR_ERR_BUSY: return "object in use";
+    default: return "unknown status";
+    }
+}
+
+const char *hicr_last_cuda_error(hicr_ctx_t *ctx) { return ctx ? ctx->cuda_error.c_str() : ""; }
+
+int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
+{
+    if (!out) return HICR_ERR_INVALID_ARG;
+    *out = nullptr;
+    int count = 0;
+    cudaError_t e = cudaGetDeviceCount(&count);
+    if (e != cudaSuccess || count == 0) {
+        (void)cudaGetLastError();
+        return HICR_ERR_CUDA;  // no CPU fallback: the product path fails loudly without a GPU
+    }
+    if (device < 0 || device >= count) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = new hicr_ctx();
+    ctx->device = device;
+    ctx->stream = static_cast<cudaStream_t>(cuda_stream);
+#define INIT_CUDA(call)                                    \
+    do {                                                   \
+        cudaError_t e__ = (call);                          \
+        if (e__ != cudaSuccess) {                          \
+            cuda_fail(ctx, e__, #call);                    \
+            fprintf(stderr, "hicr_init: %s\n", ctx->cuda_error.c_str()); \
+            hicr_finalize(ctx);                            \
+            return HICR_ERR_CUDA;                          \
+        }                                                  \
+    } while (0)
+    INIT_CUDA(cudaSetDevice(device));
+    INIT_CUDA(cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device));
+    INIT_CUDA(cudaMalloc(&ctx->d_slots, sizeof(SlotRow) * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_slots, 0xff, sizeof(SlotRow) * HICR_MAX_SLOTS));  // size = kInvalidSize
+    INIT_CUDA(cudaMalloc(&ctx->d_sent, 8 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMalloc(&ctx->d_recv, 8 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMalloc(&ctx->d_pending, 4 * 2 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_sent, 0, 8 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_recv, 0, 8 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_pending, 0, 4 * 2 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMalloc(&ctx->d_ctl, sizeof(Ctl) * kCtlRing));
+    INIT_CUDA(cudaMemset(ctx->d_ctl, 0, sizeof(Ctl) * kCtlRing));
+    ctx->h_fence_bytes = sizeof(Ctl) * kCtlRing + 2 * 8 * (size_t)HICR_MAX_SLOTS;
+    INIT_CUDA(cudaHostAlloc(&ctx->h_fence, ctx->h_fence_bytes, cudaHostAllocDefault));
+    INIT_CUDA(cudaHostAlloc(&ctx->h_call, sizeof(CallResult) * 4, cudaHostAllocMapped));
+    INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_call, ctx->h_call, 0));
+    for (int i = 0; i < 4; i++) INIT_CUDA(cudaEventCreate(&ctx->ev[i]));
+    INIT_CUDA(cudaDeviceSynchronize());
+#undef INIT_CUDA
+    *out = ctx;
+    return HICR_OK;
+}
+
+int hicr_finalize(hicr_ctx_t *ctx)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    (void)cudaSetDevice(ctx->device);
+    (void)cudaStreamSynchronize(ctx->stream);
+    cudaFree(ctx->d_slots);
+    cudaFree(ctx->d_sent);
+    cudaFree(ctx->d_recv);
+    cudaFree(ctx->d_pending);
+    cudaFree(ctx->d_ctl);
+    cudaFree(ctx->d_small);
+    cudaFree(ctx->d_chunk);
+    for (auto *v : {&ctx->free_stage, &ctx->used_stage})
+        for (auto &b : *v) {
+            cudaFreeHost(b.host);
+            cudaFree(b.dev);
+        }
+    cudaFreeHost(ctx->h_fence);
+    cudaFreeHost(ctx->h_call);
+    for (int i = 0; i < 4; i++)
+        if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
+    (void)cudaGetLastError();
+    delete ctx;
+    return HICR_OK;
+}
+
+int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_t *out)
+{
+    if (!ctx || !out) return HICR_ERR_INVALID_ARG;
+    if (!dev_ptr && size) return HICR_ERR_INVALID_ARG;
+    if (size == kInvalidSize) return HICR_ERR_INVALID_ARG;
+    if (dev_ptr) {
+        // "If the communication manager supports communication between the memory spaces
+        // ... Otherwise, it will be rejected": only this device's memory.
+        cudaPointerAttributes a;
+        cudaError_t e = cudaPointerGetAttributes(&a, dev_ptr);
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            return HICR_ERR_UNSUPPORTED_SPACE;
+        }
+        if (a.type != cudaMemoryTypeDevice || a.device != ctx->device) return HICR_ERR_UNSUPPORTED_SPACE;
+        if ((uint64_t)(uintptr_t)dev_ptr + size < (uint64_t)(uintptr_t)dev_ptr) return HICR_ERR_INVALID_ARG;
+    }
+    if (ctx->slots.size() >= HICR_MAX_SLOTS) return HICR_ERR_NO_CAPACITY;
+    SlotRow row{(uint64_t)(uintptr_t)dev_ptr, size};
+    const size_t id = ctx->slots.size();
+    // ordered after everything already enqueued on the stream; the row lives in pageable
+    // host memory, so the runtime stages it before returning
+    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + id, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->slots.push_back(row);
+    ctx->sent.push_back(0);
+    ctx->recv.push_back(0);
+    ctx->ring_refs.push_back(0);
+    ctx->registered_bytes += size;
+    *out = (hicr_slot_t)id;
+    return HICR_OK;
+}
+
+int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
+    if (ctx->ring_refs[slot]) return HICR_ERR_BUSY;
+    SlotRow row{0, kInvalidSize};
+    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + slot, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->registered_bytes -= ctx->slots[slot].size;
+    ctx->slots[slot] = row;
+    return HICR_OK;
+}
+
+int hicr_slot_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64_t *recv)
+{
+    if (!ctx || !sent || !recv) return HICR_ERR_INVALID_ARG;
+    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
+    *sent = ctx->sent[slot];
+    *recv = ctx->recv[slot];
+    return HICR_OK;
+}
+
+int hicr_fence(hicr_ctx_t *ctx)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (!ctx->epoch_open) {
+        // nothing outstanding: return at once
+        ctx->last_error = HICR_OK;
+        return HICR_OK;
+    }
+    int rc = drain_epoch(ctx, true);
+    if (rc != HICR_OK) return rc;
+    rc = ctx->epoch_error;
+    ctx->last_error = rc;
+    ctx->last_error_batch = ctx->epoch_error_batch;
+    ctx->last_error_index = ctx->epoch_error_index;
+    ctx->epoch_error = HICR_OK;
+    ctx->epoch_batch_base = 0;
+    ctx->epoch_open = false;
+    return rc;
+}
+
+int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (batch_index) *batch_index = ctx->last_error_batch;
+    if (first_bad) *first_bad = ctx->last_error_index;
+    return ctx->last_error;
+}
+
+int hicr_launch_count(hicr_ctx_t *ctx, uint64_t *launches)
+{
+    if (!ctx || !launches) return HICR_ERR_INVALID_ARG;
+    *launches = ctx->launches;
+    return HICR_OK;
+}
+
+int hicr_profile_enable(hicr_ctx_t *ctx, int on)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    ctx->profiling = on != 0;
+    ctx->ev_valid = false;
+    return HICR_OK;
+}
+
+int hicr_profile_read(hicr_ctx_t *ctx, float *ms)
+{
+    if (!ctx || !ms) return HICR_ERR_INVALID_ARG;
+    if (!ctx->ev_valid) return HICR_ERR_INVALID_ARG;
+    HICR_CUDA(ctx, cudaEventSynchronize(ctx->ev[3]));
+    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[0], ctx->ev[0], ctx->ev[1]));
+    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[1], ctx->ev[1], ctx->ev[2]));
+    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[2], ctx->ev[2], ctx->ev[3]));
+    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[3], ctx->ev[0], ctx->ev[3]));
+    return HICR_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,255 @@
+"""Parity of the channel path (hicr_channel_push / pop / stream, hicr_mpsc_stream; CUDA
+through the C-ABI) against the CPU oracle: returned counts, head/tail, ring image, sink
+image and slot message counters, bit-exact."""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from oracle import Oracle
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def hicr():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2509_01425_b200 as h
+    return h
+
+
+def _ctx(hicr):
+    return hicr.Context(0, torch.cuda.current_stream().cuda_stream)
+
+
+class Pair:
+    """The same ring / source / sink set up on the oracle and on the GPU."""
+
+    def __init__(self, hicr, T, C, src_img, sink_bytes, ring_fill=0xEE):
+        self.T, self.C = T, C
+        self.o = Oracle()
+        self.ring = np.full(T * C, ring_fill, dtype=np.uint8)
+        self.src = src_img.copy()
+        self.sink = np.zeros(sink_bytes, dtype=np.uint8)
+        self.ids = [self.o.slot_register(a) for a in (self.ring, self.src, self.sink)]
+        rc, self.och = self.o.channel_create(self.ids[0], T, C)
+        assert rc == oracle.OK
+        self.ctx = _ctx(hicr)
+        self.g = [torch.from_numpy(a.copy()).cuda() for a in (self.ring, self.src, self.sink)]
+        gids = [self.ctx.slot_register(t) for t in self.g]
+        assert gids == self.ids
+        self.ch = self.ctx.channel_create(gids[0], T, C)
+
+    def check(self, what=""):
+        torch.cuda.synchronize()
+        assert self.ch.counters() == self.o.channel_counters(self.och), what
+        for name, a, t in zip(("ring", "source", "sink"), (self.ring, self.src, self.sink), self.g):
+            assert t.cpu().numpy().tobytes() == a.tobytes(), "%s %s differs" % (what, name)
+        for s in self.ids:
+            assert self.ctx.slot_counters(s) == self.o.slot_counters(s), "%s counters of slot %d" % (what, s)
+
+    def close(self):
+        self.ctx.close()
+
+
+def test_golden_channel_examples_on_gpu(hicr, golden_dir):
+    cases = json.load(open(os.path.join(golden_dir, "channel_examples.json")))["cases"]
+    for c in cases:
+        T, C = c["token_bytes"], c["capacity"]
+        with _ctx(hicr) as ctx:
+            ring = torch.zeros(T * C, dtype=torch.uint8, device="cuda")
+            src = torch.zeros(8 * T, dtype=torch.uint8, device="cuda")
+            sink = torch.zeros(8 * T, dtype=torch.uint8, device="cuda")
+            r, s, k = ctx.slot_register(ring), ctx.slot_register(src), ctx.slot_register(sink)
+            ch = ctx.channel_create(r, T, C)
+            for op in c["ops"]:
+                if op["op"] == "push":
+                    data = np.frombuffer("".join(op["tokens"]).encode("ascii"), dtype=np.uint8).copy()
+                    src[: data.size] = torch.from_numpy(data).cuda()
+                    n = ch.push(s, 0, len(op["tokens"]))
+                else:
+                    sink.zero_()
+                    n = ch.pop(k, 0, op["max"])
+                    out = sink.cpu().numpy()
+                    assert [out[i * T: (i + 1) * T].tobytes().decode("ascii") for i in range(n)] == op["popped"], c["cite"]
+                assert n == op["returns"], c["cite"]
+                h, t = ch.counters()
+                assert h - t == op["depth"], c["cite"]
+
+
+def test_create_rejects_bad_configs(hicr):
+    with _ctx(hicr) as ctx:
+        ring = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        r = ctx.slot_register(ring)
+        for (T, C, st) in [(8, 0, hicr.HICR_ERR_INVALID_ARG), (0, 8, hicr.HICR_ERR_INVALID_ARG),
+                           (8, 9, hicr.HICR_ERR_OUT_OF_BOUNDS)]:
+            with pytest.raises(hicr.HicrError) as e:
+                ctx.channel_create(r, T, C)
+            assert e.value.status == st
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.channel_create(7, 8, 8)
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+        ch = ctx.channel_create(r, 8, 8)
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.slot_unregister(r)                      # ring still used by a live channel
+        assert e.value.status == hicr.HICR_ERR_BUSY
+        ch.close()
+        ctx.slot_unregister(r)
+
+
+@pytest.mark.parametrize("T,C", [(1, 1), (5, 3), (64, 7), (256, 16), (48, 64), (4096, 5), (33, 1024)])
+def test_random_push_pop_schedule(hicr, T, C):
+    """Random push / pop calls (including pushes into a full ring and pops from an empty
+    one): every returned count and the final state equal the oracle's."""
+    rng = np.random.default_rng(1000 + T * 7 + C)
+    n_src = 6 * C + 40
+    p = Pair(hicr, T, C, rng.integers(0, 256, n_src * T, dtype=np.uint8), n_src * T)
+    try:
+        pushed = popped = 0
+        for step in range(120):
+            if rng.random() < 0.55 and pushed < n_src:
+                n = int(rng.integers(0, min(2 * C + 2, n_src - pushed) + 1))
+                rc, k = p.o.channel_push(p.och, p.ids[1], pushed * T, n)
+                assert rc == oracle.OK
+                assert p.ch.push(p.ids[1], pushed * T, n) == k
+                pushed += k
+            else:
+                m = int(rng.integers(0, 2 * C + 2))
+                rc, k = p.o.channel_pop(p.och, p.ids[2], popped * T, m)
+                assert rc == oracle.OK
+                assert p.ch.pop(p.ids[2], popped * T, m) == k
+                popped += k
+            h, t = p.ch.counters()
+            assert (h, t) == (pushed, popped) and 0 <= h - t <= C
+        p.check("T=%d C=%d" % (T, C))
+    finally:
+        p.close()
+
+
+def test_push_pop_bounds(hicr):
+    T, C = 8, 4
+    p = Pair(hicr, T, C, np.arange(64, dtype=np.uint8), 16)
+    try:
+        with pytest.raises(hicr.HicrError) as e:
+            p.ch.push(p.ids[1], 0, 9)                    # 9 tokens = 72 B > 64 B source slot
+        assert e.value.status == oracle.ERR_OUT_OF_BOUNDS == p.o.channel_push(p.och, p.ids[1], 0, 9)[0]
+        assert p.ch.push(p.ids[1], 0, 4) == 4 == p.o.channel_push(p.och, p.ids[1], 0, 4)[1]
+        with pytest.raises(hicr.HicrError) as e:
+            p.ch.pop(p.ids[2], 0, 4)                     # 4 tokens = 32 B > 16 B sink: no effect
+        assert e.value.status == oracle.ERR_OUT_OF_BOUNDS == p.o.channel_pop(p.och, p.ids[2], 0, 4)[0]
+        assert p.ch.counters() == (4, 0)
+        assert p.ch.pop(p.ids[2], 0, 2) == 2 == p.o.channel_pop(p.och, p.ids[2], 0, 2)[1]
+        with pytest.raises(hicr.HicrError) as e:
+            p.ch.push(99, 0, 1)
+        assert e.value.status == oracle.ERR_INVALID_SLOT
+        p.check()
+    finally:
+        p.close()
+
+
+def _oracle_spsc(p, w):
+    pos = 0
+    for b in w.batches[0]:
+        assert p.o.channel_push(p.och, p.ids[1], pos * p.T, int(b)) == (oracle.OK, int(b))
+        assert p.o.channel_pop(p.och, p.ids[2], pos * p.T, p.C) == (oracle.OK, int(b))
+        pos += int(b)
+
+
+def test_config5a_host_calls_scaled(hicr):
+    """Config 5a's loop -- push(b_i) then pop(max = C) -- through the host-call path."""
+    w = W.spsc(n_tokens=30000, token_bytes=256, capacity=1024, max_batch=1024)
+    p = Pair(hicr, w.token_bytes, w.capacity, w.source_image(0), w.n_tokens * w.token_bytes)
+    try:
+        _oracle_spsc(p, w)
+        pos = 0
+        for b in w.batches[0]:
+            assert p.ch.push(p.ids[1], pos * p.T, int(b)) == int(b)
+            assert p.ch.pop(p.ids[2], pos * p.T, p.C) == int(b)
+            pos += int(b)
+        p.check("5a host calls")
+    finally:
+        p.close()
+
+
+@pytest.mark.parametrize("T,C,N,maxb", [(256, 1024, 200000, 1024), (7, 5, 3000, 9), (64, 1, 500, 3), (4096, 8, 4000, 32)])
+def test_spsc_stream_equals_call_sequence(hicr, T, C, N, maxb):
+    """hicr_channel_stream (device-resident producer and consumer in one kernel) leaves the
+    sink, ring, head/tail and message counters exactly as the oracle's push/pop sequence."""
+    w = W.spsc(n_tokens=N, token_bytes=T, capacity=C, max_batch=maxb)
+    p = Pair(hicr, T, C, w.source_image(0), N * T)
+    try:
+        # the oracle drains fully after each push; blocking pushes larger than C are split
+        pos = 0
+        for b in w.batches[0]:
+            left = int(b)
+            while left:
+                rc, k = p.o.channel_push(p.och, p.ids[1], pos * T, left)
+                assert rc == oracle.OK and k > 0
+                rc, k2 = p.o.channel_pop(p.och, p.ids[2], pos * T, C)
+                assert k2 == k
+                pos += k
+                left -= k
+        p.ch.stream(p.ids[1], 0, p.ids[2], 0, w.batches[0])
+        p.check("stream T=%d C=%d" % (T, C))
+        # and the channel is reusable by host calls afterwards, continuing the same counters
+        assert p.ch.push(p.ids[1], 0, 1) == 1 == p.o.channel_push(p.och, p.ids[1], 0, 1)[1]
+        assert p.ch.pop(p.ids[2], 0, 1) == 1 == p.o.channel_pop(p.och, p.ids[2], 0, 1)[1]
+        p.check("after stream")
+    finally:
+        p.close()
+
+
+def _mpsc_both(hicr, w, max_batch):
+    T, C, P, N = w.token_bytes, w.capacity, w.producers, w.n_tokens
+    # oracle: P independent SPSC channels driven in the seeded interleaving
+    o = Oracle()
+    rings = [np.zeros(T * C, dtype=np.uint8) for _ in range(P)]
+    srcs = [w.source_image(p) for p in range(P)]
+    sinks = [np.zeros(N * T, dtype=np.uint8) for _ in range(P)]
+    rid = [o.slot_register(a) for a in rings]
+    sid = [o.slot_register(a) for a in srcs]
+    kid = [o.slot_register(a) for a in sinks]
+    chs = [o.channel_create(rid[p], T, C)[1] for p in range(P)]
+    nxt, pushed, popped = [0] * P, [0] * P, [0] * P
+    for p in w.schedule:
+        p = int(p)
+        b = int(w.batches[p][nxt[p]])
+        nxt[p] += 1
+        done = 0
+        while done < b:
+            rc, k = o.channel_push(chs[p], sid[p], pushed[p] * T, b - done)
+            pushed[p] += k
+            done += k
+            rc, k = o.channel_pop(chs[p], kid[p], popped[p] * T, C)
+            popped[p] += k
+    with _ctx(hicr) as ctx:
+        g_r = [torch.from_numpy(a * 0).cuda() for a in rings]
+        g_s = [torch.from_numpy(a).cuda() for a in srcs]
+        g_k = [torch.zeros(N * T, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        assert [ctx.slot_register(t) for t in g_r] == rid
+        assert [ctx.slot_register(t) for t in g_s] == sid
+        assert [ctx.slot_register(t) for t in g_k] == kid
+        m = ctx.mpsc_create(rid, T, C)
+        m.stream(sid, kid, N, max_batch)
+        torch.cuda.synchronize()
+        for p in range(P):
+            assert m.counters(p) == o.channel_counters(chs[p]) == (N, N)
+            assert g_k[p].cpu().numpy().tobytes() == sinks[p].tobytes() == srcs[p].tobytes(), "sink %d" % p
+            assert g_r[p].cpu().numpy().tobytes() == rings[p].tobytes(), "ring %d" % p
+        for s in rid + sid + kid:
+            assert ctx.slot_counters(s) == o.slot_counters(s)
+
+
+@pytest.mark.parametrize("P,N,T,C,maxb", [(1, 5000, 64, 16, 16), (5, 3000, 8, 32, 48), (148, 20000, 64, 1024, 256),
+                                          (40, 1000, 100, 3, 7)])
+def test_mpsc_stream(hicr, P, N, T, C, maxb):
+    """Non-locking MPSC: one ring per producer, single consumer; per-producer
+    sink = per-producer source, head_p = tail_p = N, independent of the interleaving."""
+    w = W.mpsc(producers=P, n_tokens=N, token_bytes=T, capacity=C, max_batch=maxb)
+    _mpsc_both(hicr, w, maxb)

@@ -1,0 +1,310 @@
+"""Parity of hicr_memcpy_batch / hicr_fence (CUDA, through the C-ABI) against the CPU oracle.
+
+Bit-exact: the path is pure data movement, so every destination byte, every byte outside
+the destination ranges and every counter must equal the oracle's (north_star (d)).
+"""
+import json
+import os
+
+import numpy as np
+import pytest
+
+import workloads as W
+from parity import assert_same, run_gpu, run_oracle, to_device_table
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+
+@pytest.fixture(scope="module")
+def hicr():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2509_01425_b200 as h
+    return h
+
+
+def _ctx(hicr):
+    return hicr.Context(0, torch.cuda.current_stream().cuda_stream)
+
+
+def _bytes(s):
+    return np.frombuffer(s.encode("ascii"), dtype=np.uint8).copy()
+
+
+# ------------------------------------------------------------------ printed examples
+def test_golden_examples_on_gpu(hicr, golden_dir):
+    """The SPEC/paper printed examples (tests/golden/memcpy_examples.json), through CUDA."""
+    status = {"ok": hicr.HICR_OK, "out_of_bounds": hicr.HICR_ERR_OUT_OF_BOUNDS, "invalid_slot": hicr.HICR_ERR_INVALID_SLOT}
+    cases = json.load(open(os.path.join(golden_dir, "memcpy_examples.json")))["cases"]
+    for c in cases:
+        m = c["memcpy"]
+        overlapping = m["dst"] == m["src"] and m["size"] and \
+            m["dst_off"] < m["src_off"] + m["size"] and m["src_off"] < m["dst_off"] + m["size"]
+        if overlapping:
+            continue  # a self-overlapping copy violates the epoch precondition (reading 5)
+        with _ctx(hicr) as ctx:
+            bufs = [torch.from_numpy(_bytes(s)).cuda() if len(s) else torch.empty(0, dtype=torch.uint8, device="cuda")
+                    for s in c["slots"]]
+            ids = [ctx.slot_register(b) for b in bufs]
+            d = W.make_descs([ids[m["dst"]]], [ids[m["src"]]], [m["dst_off"]], [m["src_off"]], [m["size"]])
+            rc = hicr.HICR_OK
+            try:
+                ctx.memcpy_batch(d)
+            except hicr.HicrError as e:
+                rc = e.status
+                assert e.first_bad == 0
+            assert rc == status[c["status"]], c["cite"]
+            ctx.fence()
+            for b, e in zip(bufs, c["expect"]):
+                assert b.cpu().numpy().tobytes().decode("ascii") == e, c["cite"]
+
+
+def test_broadcast_listing_on_gpu(hicr, golden_dir):
+    """one message into N fresh slots at offset 0, a single fence."""
+    g = json.load(open(os.path.join(golden_dir, "broadcast.json")))
+    msg = _bytes(g["message"])
+    rng = np.random.default_rng(7)
+    dsts = [rng.integers(0, 256, g["destination_size"], dtype=np.uint8) for _ in range(g["n_destinations"])]
+    with _ctx(hicr) as ctx:
+        m = ctx.slot_register(torch.from_numpy(msg).cuda())
+        bufs = [torch.from_numpy(d).cuda() for d in dsts]
+        ids = [ctx.slot_register(b) for b in bufs]
+        for i in ids:
+            ctx.memcpy_batch(W.make_descs([i], [m], [0], [0], [msg.size]))
+        ctx.fence()
+        for b, d in zip(bufs, dsts):
+            out = b.cpu().numpy()
+            assert out[: msg.size].tobytes() == msg.tobytes()
+            assert out[msg.size:].tobytes() == d[msg.size:].tobytes()
+        assert ctx.slot_counters(m) == (len(ids), 0)
+        assert all(ctx.slot_counters(i) == (0, 1) for i in ids)
+
+
+# ------------------------------------------------- every alignment x ragged sizes
+SIZES = [0, 1, 2, 3, 15, 16, 17, 31, 32, 33, 47, 48, 63, 64, 65, 127, 128, 129, 255, 256, 257, 500, 511, 512, 513,
+         1023, 1024, 1025, 4095, 4096, 4097, 8191, 8192, 8193, 12345, 32767, 32768, 32769, 65535, 65536, 65537,
+         100003, 262144 + 5]
+
+
+def _alignment_workload(sizes, seed):
+    """Every (dst mod 16, src mod 16) pair for every size in ``sizes``: destinations laid
+    end to end with the wanted alignment in slot 1, sources at the wanted alignment in slot 0."""
+    rng = np.random.default_rng(seed)
+    dst_off, src_off, size = [], [], []
+    pos = 0
+    max_size = max(sizes)
+    src_bytes = max_size + 4096
+    for n in sizes:
+        for da in range(16):
+            for sa in range(16):
+                pos = (pos + 15) // 16 * 16 + da + 16 * int(rng.integers(0, 3))
+                dst_off.append(pos)
+                pos += n
+                s = int(rng.integers(0, (src_bytes - n - 16) // 16)) * 16 + sa
+                src_off.append(s)
+                size.append(n)
+    d = W.make_descs(1, 0, dst_off, src_off, size)
+    d = d[rng.permutation(len(d))]
+    w = W.CopyWorkload("alignment", 1, [src_bytes, pos + 64], [d], seed=seed)
+    return w
+
+
+@pytest.mark.parametrize("group", [0, 1, 2])
+@pytest.mark.parametrize("device_tables", [False, True])
+def test_every_alignment_and_ragged_size(hicr, group, device_tables):
+    """Brute force over head/body/tail handling: 256 alignment pairs x sizes that span the
+    byte head, the 16 B vector body (aligned and byte-shifted loads), ragged last tiles,
+    the warp-queue / chunk-queue boundary and multi-chunk descriptors."""
+    sizes = SIZES[group::3]
+    w = _alignment_workload(sizes, seed=100 + group)
+    from oracle import hazard
+    assert hazard.check(w.epochs[0], w.slot_sizes) is None
+    assert_same(w, run_oracle(w), run_gpu(w, device_tables=device_tables), "group %d" % group)
+
+
+def test_same_slot_source_and_destination(hicr):
+    """src and dst in the same slot, disjoint ranges, odd alignments (config 4's shape)."""
+    w = W.chained_epochs(n_epochs=1, n_desc=4096, slot_bytes=4 * W.MiB, smin=1, smax=700)
+    assert_same(w, run_oracle(w), run_gpu(w))
+
+
+# ------------------------------------------------------------- scaled configs 1-4
+SMALL = {
+    "tiny": lambda: W.tiny(),
+    "bulk": lambda: W.bulk_aligned(n_desc=2048, slot_bytes=64 * W.MiB, n_sets=4),
+    "heavy_a": lambda: W.heavy_tailed("a", n_slots=8, slot_bytes=16 * W.MiB, src_zone=2 * W.MiB,
+                                      n_desc=3000, smax=2 * W.MiB),
+    "heavy_b": lambda: W.heavy_tailed("b", n_slots=8, slot_bytes=16 * W.MiB, src_zone=2 * W.MiB,
+                                      n_desc=6000, smax=2 * W.MiB),
+    "chain": lambda: W.chained_epochs(n_epochs=8, n_desc=8192, slot_bytes=8 * W.MiB),
+}
+
+
+@pytest.mark.parametrize("name", sorted(SMALL))
+@pytest.mark.parametrize("device_tables", [False, True])
+def test_scaled_configs(hicr, name, device_tables):
+    w = SMALL[name]()
+    ref = run_oracle(w)
+    assert_same(w, ref, run_gpu(w, device_tables=device_tables))
+
+
+@pytest.mark.parametrize("name", ["tiny", "heavy_a"])
+def test_several_batches_one_fence(hicr, name):
+    """An epoch submitted as 7 batches before its single fence (the paper's listing issues
+    one memcpy per destination, then one fence) equals one batch.  More
+    batches than internal control blocks are covered by split=100."""
+    w = SMALL[name]()
+    ref = run_oracle(w)
+    assert_same(w, ref, run_gpu(w, split=7))
+    assert_same(w, ref, run_gpu(w, split=100, device_tables=True))
+
+
+def test_config1_counters_golden_on_gpu(hicr, golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "config1_counters.json")))
+    w = W.tiny()
+    _, per_epoch, launches = run_gpu(w)
+    assert [c[0] for c in per_epoch[-1]] == g["sent"]
+    assert [c[1] for c in per_epoch[-1]] == g["recv"]
+    assert launches > 0
+
+
+# ------------------------------------------------------------------- edge cases
+def test_zero_size_and_empty_batch(hicr):
+    with _ctx(hicr) as ctx:
+        a = torch.arange(8, dtype=torch.uint8, device="cuda")
+        b = torch.zeros(8, dtype=torch.uint8, device="cuda")
+        z = torch.empty(0, dtype=torch.uint8, device="cuda")
+        ia, ib, iz = ctx.slot_register(a), ctx.slot_register(b), ctx.slot_register(z)
+        ctx.fence()                                         # nothing outstanding: returns at once
+        ctx.memcpy_batch(np.zeros(0, dtype=hicr.DESC_DTYPE))  # n == 0 is a no-op
+        ctx.fence()
+        assert ctx.slot_counters(ia) == (0, 0)
+        # zero-size transfers move nothing and still count (reading 4); empty range at the
+        # end of a slot and on a zero-size slot are valid
+        ctx.memcpy_batch(W.make_descs([ib, ib, iz], [ia, ia, ia], [0, 8, 0], [3, 8, 2], [0, 0, 0]))
+        ctx.fence()
+        assert b.cpu().tolist() == [0] * 8
+        assert ctx.slot_counters(ia) == (3, 0) and ctx.slot_counters(ib) == (0, 2) and ctx.slot_counters(iz) == (0, 1)
+
+
+def test_rejects_non_device_memory(hicr):
+    with _ctx(hicr) as ctx:
+        host = np.zeros(64, dtype=np.uint8)
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.slot_register(int(host.ctypes.data), 64)
+        assert e.value.status == hicr.HICR_ERR_UNSUPPORTED_SPACE      # PAPER.md:373 "rejected"
+
+
+def _error_batch(kind):
+    w = W.tiny(n_desc=300, slot_bytes=64 * 1024, max_size=128)
+    d = w.epochs[0].copy()
+    if kind == "oob_dst":
+        d["dst_off"][170] = 64 * 1024 - 3
+        d["size"][170] = 4
+    elif kind == "oob_src_wrap":
+        d["src_off"][170] = 2 ** 64 - 2                               # off + size wraps u64
+        d["size"][170] = 8
+    elif kind == "bad_slot":
+        d["src_slot"][170] = 9
+    d["dst_slot"][200] = 77                                           # a later error must not win
+    return w, d
+
+
+@pytest.mark.parametrize("kind,status", [("oob_dst", "HICR_ERR_OUT_OF_BOUNDS"), ("oob_src_wrap", "HICR_ERR_OUT_OF_BOUNDS"),
+                                         ("bad_slot", "HICR_ERR_INVALID_SLOT")])
+@pytest.mark.parametrize("device_tables", [False, True])
+def test_all_or_nothing_errors(hicr, kind, status, device_tables):
+    """Reading 10: an invalid descriptor rejects the whole batch, lowest bad index reported;
+    the other batches of the epoch are unaffected.  Host tables fail at memcpy_batch,
+    device tables at the fence.  Same verdict as the oracle."""
+    from oracle import Oracle
+    w, bad = _error_batch(kind)
+    good = w.epochs[0][:100].copy()
+    imgs = [w.slot_image(0), w.slot_image(1)]
+    o = Oracle()
+    for i in imgs:
+        o.slot_register(i)
+    orc_status, orc_bad = o.memcpy_batch(bad)
+    assert orc_bad == 170
+    assert o.memcpy_batch(good)[0] == 0 and o.fence() == 0
+
+    with _ctx(hicr) as ctx:
+        bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(2)]
+        ids = [ctx.slot_register(b) for b in bufs]
+        keep = []
+        with pytest.raises(hicr.HicrError) as e:
+            if device_tables:
+                keep.append(to_device_table(good))
+                ctx.memcpy_batch(keep[-1], n=len(good))
+                keep.append(to_device_table(bad))
+                ctx.memcpy_batch(keep[-1], n=len(bad))
+                ctx.fence()
+            else:
+                ctx.memcpy_batch(good)
+                ctx.memcpy_batch(bad)
+        assert e.value.status == getattr(hicr, status) == orc_status
+        assert e.value.first_bad == 170
+        if device_tables:
+            assert e.value.batch_index == 1
+        else:
+            ctx.fence()
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == imgs[s].tobytes()
+        assert [ctx.slot_counters(s) for s in ids] == [o.slot_counters(0), o.slot_counters(1)] == [(100, 0), (0, 100)]
+        # the context keeps working after a rejected batch
+        ctx.memcpy_batch(w.epochs[0][100:200].copy())
+        ctx.fence()
+        assert ctx.slot_counters(0) == (200, 0)
+
+
+def test_unregister_then_use_is_invalid_slot(hicr):
+    with _ctx(hicr) as ctx:
+        a = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        b = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        ia, ib = ctx.slot_register(a), ctx.slot_register(b)
+        ctx.slot_unregister(ia)
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.slot_unregister(ia)
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.memcpy_batch(W.make_descs([ib], [ia], [0], [0], [8]))
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+        t = to_device_table(W.make_descs([ib], [ia], [0], [0], [8]))
+        ctx.memcpy_batch(t, n=1)
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence()
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+
+
+# ------------------------------------------------------------ full-size configs
+def test_config2_full_size(hicr):
+    """BASELINE.json config 2 at full size (2 x 1 GiB, 4 x 65,536 x 4 KiB), in the launch
+    configuration bench.py times (device-resident tables, one batch + one fence per set)."""
+    w = W.bulk_aligned()
+    ref = run_oracle(w)
+    got = run_gpu(w, device_tables=True)
+    assert_same(w, ref, got)
+    assert got[1][-1] == [(4 * 65536, 0), (0, 4 * 65536)]
+
+
+def test_config4_full_size(hicr):
+    """BASELINE.json config 4 at full size: 64 fence epochs x 65,536 descriptors on one
+    256 MiB slot; final image and per-epoch counters."""
+    w = W.chained_epochs()
+    ref = run_oracle(w)
+    got = run_gpu(w, device_tables=True)
+    assert_same(w, ref, got)
+    for k, c in enumerate(got[1]):
+        assert c == [(65536 * (k + 1), 65536 * (k + 1))]
+
+
+@pytest.mark.parametrize("variant", ["a", "b"])
+def test_config3_quarter_size(hicr, variant):
+    """Config 3's size law and alignment mix at a quarter of the slot count (16 x 256 MiB =
+    4 GiB, 25,000 descriptors, sizes up to 16 MiB), whole-image parity."""
+    w = W.heavy_tailed(variant, n_slots=16, n_desc=25000)
+    ref = run_oracle(w)
+    got = run_gpu(w, device_tables=True)
+    assert_same(w, ref, got)
