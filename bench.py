@@ -332,8 +332,9 @@ def run_cuda(args):
     if rank == 0:
         peak, peak_src = load_peaks()
         prof /= max(1, n_prof)
-        kernel_ms = {"plan": prof[0], "copy_warp": prof[1], "copy_cta": prof[2], "all": prof[3]}
-        dom = "copy_warp" if prof[1] >= prof[2] else "copy_cta"
+        kernel_ms = {"plan_phase": prof[0], "copy_phase": prof[1], "engine_kernel_globaltimer": prof[2],
+                     "engine_kernel": prof[3]}
+        dom = "engine_kernel"          # the one kernel of a step; duration from CUDA events around its launch
         achieved = bps / (kernel_ms[dom] * 1e-3) / 1e9 if kernel_ms[dom] > 0 else 0.0
         traffic = None
         tp = os.path.join(ROOT, "profiles", "traffic.json")
@@ -364,7 +365,7 @@ def run_cuda(args):
                     "ms_per_step": agg_e2e["ms_per_step"], "what": "host descriptor tables in, slot counters out"},
             "gpu_launches": int(launches),
             "kernel_ms": kernel_ms,
-            "roofline": {"bound": "hbm", "kernel": dom + "_kernel", "achieved": achieved, "peak": peak, "unit": UNIT,
+            "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": UNIT,
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
                          "algorithmic_bytes_per_launch": bps},
             "cpu_baseline": cpu,

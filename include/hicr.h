@@ -205,11 +205,11 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_sl
 /* Kernel launches issued by this context since hicr_init (host pointer out). */
 int hicr_launch_count(hicr_ctx_t *ctx, uint64_t *launches);
 
-/* With profiling on, every hicr_memcpy_batch records CUDA events around its kernels on
- * the context's stream.  hicr_profile_read (after a fence) returns, for the LAST batch,
- * the device time in milliseconds of: [0] the plan/binning kernel, [1] the warp-per-
- * descriptor copy kernel, [2] the CTA-per-chunk copy kernel, [3] all three end to end.
- * ms: host pointer to 4 floats. */
+/* With profiling on, every hicr_memcpy_batch records CUDA events around its engine kernel
+ * on the context's stream.  hicr_profile_read (only right after a fence) returns, for the
+ * LAST batch, in milliseconds: [0] the validation/binning phase up to the grid barrier and
+ * [1] the copy phase, both from the device's %globaltimer stamps in the completion record,
+ * [2] their sum, [3] the whole kernel from the CUDA events.  ms: host pointer to 4 floats. */
 int hicr_profile_enable(hicr_ctx_t *ctx, int on);
 int hicr_profile_read(hicr_ctx_t *ctx, float *ms);
 

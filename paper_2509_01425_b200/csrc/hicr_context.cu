@@ -30,13 +30,12 @@ static int bad_to_status(unsigned id)
     }
 }
 
-// Read back the slot counters (device -> pinned -> host mirror).  Stream must be idle or
-// the caller synchronizes afterwards; here we synchronize.
+// Read back the slot counters (device -> pinned -> host mirror) and wait for the stream.
 int refresh_counters(hicr_ctx *ctx)
 {
     const size_t n = ctx->slots.size();
     if (n == 0) return HICR_OK;
-    unsigned char *p = ctx->h_fence + sizeof(Ctl) * kCtlRing;
+    unsigned char *p = ctx->h_fence;
     HICR_CUDA(ctx, cudaMemcpyAsync(p, ctx->d_sent, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
     HICR_CUDA(ctx, cudaMemcpyAsync(p + 8 * (size_t)HICR_MAX_SLOTS, ctx->d_recv, n * 8, cudaMemcpyDeviceToHost,
                                    ctx->stream));
@@ -46,28 +45,46 @@ int refresh_counters(hicr_ctx *ctx)
     return HICR_OK;
 }
 
-// Complete everything enqueued so far in this epoch: copy the used control blocks and
-// the counters back, wait, fold deferred errors into the epoch state, reset the control
-// blocks and recycle staging.  final_fence distinguishes hicr_fence from the internal
-// drain that happens when an epoch issues more than kCtlRing batches.
+// Wait until the engine kernel of batch `seq` has published its completion record `r`
+// (mapped pinned memory).  Polls the record; every so often asks the stream, so that a
+// faulted kernel turns into HICR_ERR_CUDA instead of a hang.
+static int wait_record(hicr_ctx *ctx, const HostRecord *r, uint64_t seq)
+{
+    const volatile unsigned long long *flag = &r->seq;
+    for (unsigned spins = 0;; spins++) {
+        if (*flag == seq) break;
+        if ((spins & 0x3fff) == 0x3fff) {
+            cudaError_t e = cudaStreamQuery(ctx->stream);
+            if (e == cudaSuccess) {
+                if (*flag == seq) break;
+                ctx->cuda_error = "engine kernel finished without publishing its completion record";
+                return HICR_ERR_CUDA;
+            }
+            if (e != cudaErrorNotReady) return cuda_fail(ctx, e, "cudaStreamQuery(fence)");
+        }
+    }
+    __atomic_thread_fence(__ATOMIC_ACQUIRE);
+    return HICR_OK;
+}
+
+// Complete everything enqueued so far in this epoch: wait for the last batch's completion
+// record (stream order makes the earlier ones complete too), fold deferred errors into the
+// epoch state, take the pushed counters and recycle staging.  final_fence distinguishes
+// hicr_fence from the internal drain that happens when an epoch issues more than kRecRing
+// batches.
 int drain_epoch(hicr_ctx *ctx, bool final_fence)
 {
     const uint32_t nb = ctx->batches_in_epoch;
     const size_t n = ctx->slots.size();
-    unsigned char *p = ctx->h_fence;
-    if (nb) HICR_CUDA(ctx, cudaMemcpyAsync(p, ctx->d_ctl, sizeof(Ctl) * nb, cudaMemcpyDeviceToHost, ctx->stream));
-    unsigned char *pc = p + sizeof(Ctl) * kCtlRing;
-    if (n && final_fence) {
-        HICR_CUDA(ctx, cudaMemcpyAsync(pc, ctx->d_sent, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
-        HICR_CUDA(ctx, cudaMemcpyAsync(pc + 8 * (size_t)HICR_MAX_SLOTS, ctx->d_recv, n * 8, cudaMemcpyDeviceToHost,
-                                       ctx->stream));
+    if (nb) {
+        int rc = wait_record(ctx, ctx->h_rec + (nb - 1), ctx->batch_seq);
+        if (rc != HICR_OK) return rc;
+        ctx->last_rec = ctx->h_rec[nb - 1];
     }
-    if (nb) HICR_CUDA(ctx, cudaMemsetAsync(ctx->d_ctl, 0, sizeof(Ctl) * nb, ctx->stream));
-    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    const Ctl *c = reinterpret_cast<const Ctl *>(p);
     for (uint32_t b = 0; b < nb; b++) {
-        if (c[b].bad_inv != 0 && ctx->epoch_error == HICR_OK) {
-            const unsigned long long packed = ~c[b].bad_inv;
+        const unsigned long long bad_inv = ctx->h_rec[b].bad_inv;
+        if (bad_inv != 0 && ctx->epoch_error == HICR_OK) {
+            const unsigned long long packed = ~bad_inv;
             ctx->epoch_error = bad_to_status((unsigned)(packed & 15));
             ctx->epoch_error_batch = ctx->epoch_batch_base + b;
             ctx->epoch_error_index = packed >> 4;
@@ -76,8 +93,15 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence)
     ctx->epoch_batch_base += nb;
     ctx->batches_in_epoch = 0;
     if (n && final_fence) {
-        memcpy(ctx->sent.data(), pc, n * 8);
-        memcpy(ctx->recv.data(), pc + 8 * (size_t)HICR_MAX_SLOTS, n * 8);
+        if (nb && n <= kPushSlots) {
+            // the last batch pushed the cumulative counters next to the records
+            const unsigned long long *push = reinterpret_cast<const unsigned long long *>(ctx->h_rec + kRecRing);
+            memcpy(ctx->sent.data(), push, n * 8);
+            memcpy(ctx->recv.data(), push + kPushSlots, n * 8);
+        } else {
+            int rc = refresh_counters(ctx);
+            if (rc != HICR_OK) return rc;
+        }
     }
     for (auto &b : ctx->used_stage) ctx->free_stage.push_back(b);
     ctx->used_stage.clear();
@@ -137,19 +161,31 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
     INIT_CUDA(cudaMemset(ctx->d_slots, 0xff, sizeof(SlotRow) * HICR_MAX_SLOTS));  // size = kInvalidSize
     INIT_CUDA(cudaMalloc(&ctx->d_sent, 8 * HICR_MAX_SLOTS));
     INIT_CUDA(cudaMalloc(&ctx->d_recv, 8 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMalloc(&ctx->d_pending, 4 * 2 * HICR_MAX_SLOTS));
     INIT_CUDA(cudaMemset(ctx->d_sent, 0, 8 * HICR_MAX_SLOTS));
     INIT_CUDA(cudaMemset(ctx->d_recv, 0, 8 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMemset(ctx->d_pending, 0, 4 * 2 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMalloc(&ctx->d_ctl, sizeof(Ctl) * kCtlRing));
-    INIT_CUDA(cudaMemset(ctx->d_ctl, 0, sizeof(Ctl) * kCtlRing));
-    ctx->h_fence_bytes = sizeof(Ctl) * kCtlRing + 2 * 8 * (size_t)HICR_MAX_SLOTS;
+    INIT_CUDA(cudaMalloc(&ctx->d_ctl, sizeof(Ctl)));
+    INIT_CUDA(cudaMemset(ctx->d_ctl, 0, sizeof(Ctl)));
+    {
+        const size_t rec_bytes = sizeof(HostRecord) * kRecRing + 2 * 8 * (size_t)kPushSlots;
+        INIT_CUDA(cudaHostAlloc(&ctx->h_rec, rec_bytes, cudaHostAllocMapped));
+        memset(ctx->h_rec, 0, rec_bytes);
+        INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_rec, ctx->h_rec, 0));
+    }
+    ctx->h_fence_bytes = 2 * 8 * (size_t)HICR_MAX_SLOTS;
     INIT_CUDA(cudaHostAlloc(&ctx->h_fence, ctx->h_fence_bytes, cudaHostAllocDefault));
     INIT_CUDA(cudaHostAlloc(&ctx->h_call, sizeof(CallResult) * 4, cudaHostAllocMapped));
     INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_call, ctx->h_call, 0));
-    for (int i = 0; i < 4; i++) INIT_CUDA(cudaEventCreate(&ctx->ev[i]));
+    for (int i = 0; i < 2; i++) INIT_CUDA(cudaEventCreate(&ctx->ev[i]));
     INIT_CUDA(cudaDeviceSynchronize());
 #undef INIT_CUDA
+    {
+        int rc = engine_setup(ctx);
+        if (rc != HICR_OK) {
+            fprintf(stderr, "hicr_init: engine kernel cannot be made resident: %s\n", ctx->cuda_error.c_str());
+            hicr_finalize(ctx);
+            return rc;
+        }
+    }
     *out = ctx;
     return HICR_OK;
 }
@@ -162,7 +198,6 @@ int hicr_finalize(hicr_ctx_t *ctx)
     cudaFree(ctx->d_slots);
     cudaFree(ctx->d_sent);
     cudaFree(ctx->d_recv);
-    cudaFree(ctx->d_pending);
     cudaFree(ctx->d_ctl);
     cudaFree(ctx->d_small);
     cudaFree(ctx->d_chunk);
@@ -172,8 +207,9 @@ int hicr_finalize(hicr_ctx_t *ctx)
             cudaFree(b.dev);
         }
     cudaFreeHost(ctx->h_fence);
+    cudaFreeHost(ctx->h_rec);
     cudaFreeHost(ctx->h_call);
-    for (int i = 0; i < 4; i++)
+    for (int i = 0; i < 2; i++)
         if (ctx->ev[i]) cudaEventDestroy(ctx->ev[i]);
     (void)cudaGetLastError();
     delete ctx;
@@ -279,12 +315,13 @@ int hicr_profile_enable(hicr_ctx_t *ctx, int on)
 int hicr_profile_read(hicr_ctx_t *ctx, float *ms)
 {
     if (!ctx || !ms) return HICR_ERR_INVALID_ARG;
-    if (!ctx->ev_valid) return HICR_ERR_INVALID_ARG;
-    HICR_CUDA(ctx, cudaEventSynchronize(ctx->ev[3]));
-    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[0], ctx->ev[0], ctx->ev[1]));
-    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[1], ctx->ev[1], ctx->ev[2]));
-    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[2], ctx->ev[2], ctx->ev[3]));
-    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[3], ctx->ev[0], ctx->ev[3]));
+    if (!ctx->ev_valid || ctx->epoch_open) return HICR_ERR_INVALID_ARG;   // only after a fence
+    const HostRecord &r = ctx->last_rec;
+    ms[0] = (float)((double)(r.t_mid - r.t_start) * 1e-6);
+    ms[1] = (float)((double)(r.t_end - r.t_mid) * 1e-6);
+    ms[2] = (float)((double)(r.t_end - r.t_start) * 1e-6);
+    HICR_CUDA(ctx, cudaEventSynchronize(ctx->ev[1]));
+    HICR_CUDA(ctx, cudaEventElapsedTime(&ms[3], ctx->ev[0], ctx->ev[1]));
     return HICR_OK;
 }
 

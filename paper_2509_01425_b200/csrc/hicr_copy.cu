@@ -1,24 +1,33 @@
 // hicr_copy.cu -- hicr_memcpy_batch: descriptor ingest + validation (a2), binning and
-// work expansion (a3), the two copy kernels (a4, a5) and counter accumulation (a6).
+// work expansion (a3), the copies (a4, a5) and counter accumulation (a6), as ONE
+// persistent cooperative kernel per batch.
 //
 // The operation: the Communication Manager's memcpy, "specify the source and
 // destination memory slots, as well as the offsets within them and the size of data to
 // communicate ... the operation will be initiated. Otherwise, it will be rejected"
 // (PAPER.md:373), batched; completion deferred to the fence.
 //
-// Per batch, on the context's stream:
-//   plan_kernel        one thread per descriptor: validate against the slot table, resolve
-//                      absolute addresses, classify by size, compact into the warp queue /
-//                      expand into the chunk queue (warp ballot + warp prefix sums + one
-//                      atomic per warp per queue), aggregate the per-slot message counts;
-//                      the last CTA to finish commits the batch (go = 1, counts folded into
-//                      the cumulative counters) iff no descriptor was invalid.
-//   copy_small_kernel  persistent, one warp per queued descriptor of <= kSmallMax bytes.
-//   copy_chunk_kernel  persistent, one CTA per kChunkBytes chunk of a larger descriptor.
-// Both copy kernels do nothing unless go == 1, which makes the batch all-or-nothing.
+// engine_kernel, grid = SMs x kCtasPerSm co-resident CTAs of 256 threads:
+//   phase A  one thread per descriptor (grid-stride tiles): validate against the slot
+//            table, resolve absolute addresses, classify by size, compact into the warp
+//            queue / expand into the chunk queue (warp ballot + warp prefix sums + one
+//            atomic per warp per queue), count messages per slot in a shared-memory
+//            histogram.
+//   barrier  grid-wide (one atomic per CTA); afterwards every CTA knows whether any
+//            descriptor was invalid.  If so nothing is copied or counted: all-or-nothing.
+//   phase B  histogram flushed into the cumulative u64 counters (one atomic per touched
+//            slot per CTA); then dynamic work tickets (one atomic per CTA per ticket,
+//            prefetched one round ahead): a ticket is one chunk (CTA-per-chunk) or eight
+//            small descriptors (warp-per-descriptor).  16 B-aligned spans of at least
+//            tma_min bytes go through 1-D TMA bulk copies staged in shared memory, one
+//            4 KiB stage per warp; everything else through 16 B vector loads / aligned
+//            stores with byte-shifted sources (copy_span).
+//   finish   the last CTA to finish pushes the counters and the completion record into
+//            mapped pinned host memory (what hicr_fence polls) and clears the control block.
 #include "hicr_internal.cuh"
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 
 namespace hicr {
@@ -28,147 +37,25 @@ __device__ __forceinline__ void report_bad(Ctl *ctl, uint64_t index, unsigned id
     atomicMax(&ctl->bad_inv, ~((unsigned long long)index << 4 | id));
 }
 
-// (a2) + (a3) + (a6)
-__global__ void __launch_bounds__(kPlanThreads)
-plan_kernel(const hicr_desc_t *__restrict__ descs, uint64_t n, const SlotRow *__restrict__ slots, uint32_t n_slots,
-            Ctl *ctl, WorkItem *__restrict__ small_q, uint64_t small_cap, WorkItem *__restrict__ chunk_q,
-            uint64_t chunk_cap, unsigned int *pending, unsigned long long *sent, unsigned long long *recv)
+__device__ __forceinline__ unsigned long long globaltimer()
 {
-    extern __shared__ unsigned int hist[];  // [2 * n_slots] when n_slots <= kSmemSlotHist
-    const bool use_hist = n_slots <= kSmemSlotHist;
-    if (use_hist) {
-        for (uint32_t i = threadIdx.x; i < 2 * n_slots; i += blockDim.x) hist[i] = 0;
-        __syncthreads();
-    }
-    const int lane = threadIdx.x & 31;
-    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
-    const bool active = i < n;
+    unsigned long long t;
+    asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+    return t;
+}
 
-    uint64_t src = 0, dst = 0, size = 0;
-    uint32_t ss = 0, ds = 0;
-    bool valid = false;
-    if (active) {
-        const uint4 *p = reinterpret_cast<const uint4 *>(descs + i);
-        const uint4 lo = __ldg(p), hi = __ldg(p + 1);
-        ds = lo.x;
-        ss = lo.y;
-        const uint64_t dst_off = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
-        const uint64_t src_off = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
-        size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
-        // destination checked before source; overflow-safe "off + size <= slot size"
-        unsigned bad = 0;
-        SlotRow dr{0, kInvalidSize}, sr{0, kInvalidSize};
-        if (ds < n_slots) dr = slots[ds];
-        if (ss < n_slots) sr = slots[ss];
-        if (dr.size == kInvalidSize) bad = kBadInvalidSlot;
-        else if (dst_off > dr.size || size > dr.size - dst_off) bad = kBadOutOfBounds;
-        else if (sr.size == kInvalidSize) bad = kBadInvalidSlot;
-        else if (src_off > sr.size || size > sr.size - src_off) bad = kBadOutOfBounds;
-        if (bad) report_bad(ctl, i, bad);
-        else {
-            valid = true;
-            dst = dr.base + dst_off;
-            src = sr.base + src_off;
-        }
-    }
+__device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
+{
+    unsigned v;
+    asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 
-    // ---- (a6) one message per descriptor: sent on the source slot, recv on the destination
-    // (lanes with the same slot elect one leader; invalid lanes carry a key no slot has)
-    {
-        const unsigned ms = __match_any_sync(0xffffffffu, valid ? ss : 0xffffffffu);
-        if (valid && lane == __ffs(ms) - 1) {
-            if (use_hist) atomicAdd(&hist[ss], __popc(ms)); else atomicAdd(&pending[ss], __popc(ms));
-        }
-        const unsigned md = __match_any_sync(0xffffffffu, valid ? ds : 0xffffffffu);
-        if (valid && lane == __ffs(md) - 1) {
-            if (use_hist) atomicAdd(&hist[n_slots + ds], __popc(md));
-            else atomicAdd(&pending[HICR_MAX_SLOTS + ds], __popc(md));
-        }
-    }
-
-    // ---- (a3) binning: warp ballot + prefix sums, one atomic per warp per queue
-    const bool is_small = valid && size <= kSmallMax;   // zero-size descriptors move nothing
-    const bool is_large = valid && size > kSmallMax;
-    const unsigned small_mask = __ballot_sync(0xffffffffu, is_small && size > 0);
-    if (small_mask) {
-        unsigned base = 0;
-        if (lane == 0) base = atomicAdd(&ctl->n_small, __popc(small_mask));
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (is_small && size > 0) {
-            const uint64_t pos = base + __popc(small_mask & ((1u << lane) - 1));
-            if (pos < small_cap) {
-                uint4 *q = reinterpret_cast<uint4 *>(small_q + pos);
-                q[0] = make_uint4((unsigned)src, (unsigned)(src >> 32), (unsigned)dst, (unsigned)(dst >> 32));
-                q[1] = make_uint4((unsigned)size, (unsigned)(size >> 32), 0, 0);
-            } else report_bad(ctl, i, kBadNoCapacity);
-        }
-    }
-    const unsigned large_mask = __ballot_sync(0xffffffffu, is_large);
-    if (large_mask) {
-        const unsigned nch = is_large ? (unsigned)((size + kChunkBytes - 1) / kChunkBytes) : 0u;
-        // inclusive warp scan of the chunk counts
-        unsigned incl = nch;
-#pragma unroll
-        for (int d = 1; d < 32; d <<= 1) {
-            const unsigned v = __shfl_up_sync(0xffffffffu, incl, d);
-            if (lane >= d) incl += v;
-        }
-        const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
-        unsigned base = 0;
-        if (lane == 0) base = atomicAdd(&ctl->n_chunk, total);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        const uint64_t my_first = (uint64_t)base + (incl - nch);
-        if (is_large && my_first + nch > chunk_cap) report_bad(ctl, i, kBadNoCapacity);
-        // work expansion: the whole warp writes the chunk items of each large descriptor
-        unsigned m = large_mask;
-        while (m) {
-            const int l = __ffs(m) - 1;
-            m &= m - 1;
-            const uint64_t s0 = __shfl_sync(0xffffffffu, src, l);
-            const uint64_t d0 = __shfl_sync(0xffffffffu, dst, l);
-            const uint64_t sz = __shfl_sync(0xffffffffu, size, l);
-            const uint64_t first = __shfl_sync(0xffffffffu, my_first, l);
-            const unsigned cnt = __shfl_sync(0xffffffffu, nch, l);
-            if (first + cnt > chunk_cap) continue;
-            for (unsigned c = lane; c < cnt; c += 32) {
-                const uint64_t off = (uint64_t)c * kChunkBytes;
-                const uint64_t len = min(kChunkBytes, sz - off);
-                uint4 *q = reinterpret_cast<uint4 *>(chunk_q + first + c);
-                const uint64_t s1 = s0 + off, d1 = d0 + off;
-                q[0] = make_uint4((unsigned)s1, (unsigned)(s1 >> 32), (unsigned)d1, (unsigned)(d1 >> 32));
-                q[1] = make_uint4((unsigned)len, (unsigned)(len >> 32), 0, 0);
-            }
-        }
-    }
-
-    // ---- flush the CTA histogram, then the last CTA commits or discards the batch
-    if (use_hist) {
-        __syncthreads();
-        for (uint32_t s = threadIdx.x; s < 2 * n_slots; s += blockDim.x) {
-            const unsigned v = hist[s];
-            if (v) atomicAdd(&pending[s < n_slots ? s : HICR_MAX_SLOTS + (s - n_slots)], v);
-        }
-    }
-    __threadfence();
-    __syncthreads();
-    __shared__ bool last;
-    if (threadIdx.x == 0) last = atomicAdd(&ctl->done, 1u) == gridDim.x - 1;
-    __syncthreads();
-    if (!last) return;
-    __threadfence();
-    const bool ok = *reinterpret_cast<volatile unsigned long long *>(&ctl->bad_inv) == 0;
-    for (uint32_t s = threadIdx.x; s < n_slots; s += blockDim.x) {
-        const unsigned a = __ldcg(&pending[s]), b = __ldcg(&pending[HICR_MAX_SLOTS + s]);
-        if (a) {
-            if (ok) sent[s] += a;
-            pending[s] = 0;
-        }
-        if (b) {
-            if (ok) recv[s] += b;
-            pending[HICR_MAX_SLOTS + s] = 0;
-        }
-    }
-    if (threadIdx.x == 0) ctl->go = ok ? 1u : 0u;
+__device__ __forceinline__ void put_item(WorkItem *q, uint64_t src, uint64_t dst, uint64_t size)
+{
+    uint4 *p = reinterpret_cast<uint4 *>(q);
+    p[0] = make_uint4((unsigned)src, (unsigned)(src >> 32), (unsigned)dst, (unsigned)(dst >> 32));
+    p[1] = make_uint4((unsigned)size, (unsigned)(size >> 32), 0, 0);
 }
 
 __device__ __forceinline__ WorkItem load_item(const WorkItem *q)
@@ -183,40 +70,277 @@ __device__ __forceinline__ WorkItem load_item(const WorkItem *q)
     return w;
 }
 
-// (a4) one warp per descriptor of <= kSmallMax bytes
-__global__ void __launch_bounds__(kCopyThreads)
-copy_small_kernel(const Ctl *__restrict__ ctl, const WorkItem *__restrict__ q)
+// Chunks of a large descriptor.  From kAlignedSplitMin bytes on, the cuts sit at multiples of
+// kChunkBytes of the DESTINATION address, so every chunk but the first starts 16 B-aligned
+// (no byte head, and TMA-eligible when the source is congruent); below that, every
+// kChunkBytes from the start.
+constexpr uint64_t kAlignedSplitMin = 4 * kChunkBytes;
+__device__ __forceinline__ unsigned chunk_count(uint64_t dst, uint64_t size)
 {
-    if (__ldcg(&ctl->go) == 0) return;
-    const unsigned n = __ldcg(&ctl->n_small);
-    const int lane = threadIdx.x & 31;
-    const unsigned warps = gridDim.x * (kCopyThreads / 32);
-    unsigned i = blockIdx.x * (kCopyThreads / 32) + (threadIdx.x >> 5);
-    if (i >= n) return;
-    WorkItem w = load_item(q + i);
-    while (true) {
-        const unsigned nxt = i + warps;
-        WorkItem wn;
-        if (nxt < n) wn = load_item(q + nxt);   // fetch the next item while this one is copied
-        copy_span<kUnroll, kLdStream>(reinterpret_cast<unsigned char *>(w.dst),
-                                      reinterpret_cast<const unsigned char *>(w.src), w.size, lane, 32);
-        if (nxt >= n) break;
-        w = wn;
-        i = nxt;
+    if (size >= kAlignedSplitMin) return (unsigned)((dst + size - 1) / kChunkBytes - dst / kChunkBytes + 1);
+    return (unsigned)((size + kChunkBytes - 1) / kChunkBytes);
+}
+__device__ __forceinline__ void chunk_range(uint64_t dst, uint64_t size, unsigned c, uint64_t &off, uint64_t &len)
+{
+    if (size >= kAlignedSplitMin) {
+        const uint64_t first = dst / kChunkBytes;
+        const uint64_t lo = c == 0 ? dst : (first + c) * kChunkBytes;
+        const uint64_t hi = min(dst + size, (first + c + 1) * kChunkBytes);
+        off = lo - dst;
+        len = hi - lo;
+    } else {
+        off = (uint64_t)c * kChunkBytes;
+        len = min(kChunkBytes, size - off);
     }
 }
 
-// (a5) one CTA per chunk of a large descriptor
-__global__ void __launch_bounds__(kCopyThreads)
-copy_chunk_kernel(const Ctl *__restrict__ ctl, const WorkItem *__restrict__ q)
+struct EngineArgs {
+    const hicr_desc_t *descs;
+    uint64_t n;
+    const SlotRow *slots;
+    uint32_t n_slots;
+    uint32_t tma_min;
+    Ctl *ctl;
+    WorkItem *small_q;
+    uint64_t small_cap;
+    WorkItem *chunk_q;
+    uint64_t chunk_cap;
+    unsigned long long *sent;
+    unsigned long long *recv;
+    HostRecord *rec;                 // this batch's record (device alias of mapped pinned memory)
+    unsigned long long *push;        // [2 * kPushSlots] pushed counters (device alias of mapped pinned memory)
+    uint32_t n_push;
+    uint32_t pad;
+    unsigned long long seq;
+};
+
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const EngineArgs a)
 {
-    if (__ldcg(&ctl->go) == 0) return;
-    const unsigned n = __ldcg(&ctl->n_chunk);
-    for (unsigned i = blockIdx.x; i < n; i += gridDim.x) {
-        const WorkItem w = load_item(q + i);
-        copy_span<kUnroll, kLdStream>(reinterpret_cast<unsigned char *>(w.dst),
-                                      reinterpret_cast<const unsigned char *>(w.src), w.size, threadIdx.x,
-                                      kCopyThreads);
+    extern __shared__ __align__(128) unsigned char dyn_smem[];   // [kWarps x kTmaPiece stages][histogram]
+    __shared__ uint64_t bars[kWarps];
+    __shared__ unsigned sh_ticket[2];
+    __shared__ unsigned sh_flag;
+    unsigned int *hist = reinterpret_cast<unsigned int *>(dyn_smem + (size_t)kWarps * kTmaPiece);
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    Ctl *ctl = a.ctl;
+    const uint32_t n_slots = a.n_slots;
+    const bool use_hist = n_slots <= kSmemSlotHist;
+    if (blockIdx.x == 0 && tid == 0) ctl->t_start = globaltimer();
+    if (use_hist)
+        for (uint32_t i = tid; i < 2 * n_slots; i += kThreads) hist[i] = 0;
+    TmaLane tma;
+    tma.stage = dyn_smem + (size_t)warp * kTmaPiece;
+    tma.bar = &bars[warp];
+    tma.phase = 0;
+    tma.pending = false;
+    if (lane == 0) {
+        mbar_init(tma.bar, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // ================================================================ phase A (a2, a3, a6)
+    for (uint64_t tile = (uint64_t)blockIdx.x * kThreads; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
+        const uint64_t i = tile + tid;
+        const bool active = i < a.n;
+        uint64_t src = 0, dst = 0, size = 0;
+        uint32_t ss = 0, ds = 0;
+        bool valid = false;
+        if (active) {
+            const uint4 *p = reinterpret_cast<const uint4 *>(a.descs + i);
+            const uint4 lo = __ldg(p), hi = __ldg(p + 1);
+            ds = lo.x;
+            ss = lo.y;
+            const uint64_t dst_off = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
+            const uint64_t src_off = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+            size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
+            // destination checked before source; overflow-safe "off + size <= slot size"
+            unsigned bad = 0;
+            SlotRow dr{0, kInvalidSize}, sr{0, kInvalidSize};
+            if (ds < n_slots) dr = a.slots[ds];
+            if (ss < n_slots) sr = a.slots[ss];
+            if (dr.size == kInvalidSize) bad = kBadInvalidSlot;
+            else if (dst_off > dr.size || size > dr.size - dst_off) bad = kBadOutOfBounds;
+            else if (sr.size == kInvalidSize) bad = kBadInvalidSlot;
+            else if (src_off > sr.size || size > sr.size - src_off) bad = kBadOutOfBounds;
+            if (bad) report_bad(ctl, i, bad);
+            else {
+                valid = true;
+                dst = dr.base + dst_off;
+                src = sr.base + src_off;
+            }
+        }
+
+        // ---- (a6) one message per descriptor: sent on the source slot, recv on the destination
+        // (lanes with the same slot elect one leader; invalid lanes carry a key no slot has)
+        if (use_hist) {
+            const unsigned ms = __match_any_sync(0xffffffffu, valid ? ss : 0xffffffffu);
+            if (valid && lane == __ffs(ms) - 1) atomicAdd(&hist[ss], __popc(ms));
+            const unsigned md = __match_any_sync(0xffffffffu, valid ? ds : 0xffffffffu);
+            if (valid && lane == __ffs(md) - 1) atomicAdd(&hist[n_slots + ds], __popc(md));
+        }
+
+        // ---- (a3) binning: warp ballot + prefix sums, one atomic per warp per queue
+        const bool is_small = valid && size <= kSmallMax && size > 0;   // zero-size descriptors move nothing
+        const bool is_large = valid && size > kSmallMax;
+        const unsigned small_mask = __ballot_sync(0xffffffffu, is_small);
+        if (small_mask) {
+            unsigned base = 0;
+            if (lane == 0) base = atomicAdd(&ctl->n_small, __popc(small_mask));
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if (is_small) {
+                const uint64_t pos = base + __popc(small_mask & ((1u << lane) - 1));
+                if (pos < a.small_cap) put_item(a.small_q + pos, src, dst, size);
+                else report_bad(ctl, i, kBadNoCapacity);
+            }
+        }
+        const unsigned large_mask = __ballot_sync(0xffffffffu, is_large);
+        if (large_mask) {
+            const unsigned nch = is_large ? chunk_count(dst, size) : 0u;
+            unsigned incl = nch;   // inclusive warp scan of the chunk counts
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned v = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += v;
+            }
+            const unsigned total = __shfl_sync(0xffffffffu, incl, 31);
+            unsigned base = 0;
+            if (lane == 0) base = atomicAdd(&ctl->n_chunk, total);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            const uint64_t my_first = (uint64_t)base + (incl - nch);
+            if (is_large && my_first + nch > a.chunk_cap) report_bad(ctl, i, kBadNoCapacity);
+            // work expansion: the whole warp writes the chunk items of each large descriptor
+            unsigned m = large_mask;
+            while (m) {
+                const int l = __ffs(m) - 1;
+                m &= m - 1;
+                const uint64_t s0 = __shfl_sync(0xffffffffu, src, l);
+                const uint64_t d0 = __shfl_sync(0xffffffffu, dst, l);
+                const uint64_t sz = __shfl_sync(0xffffffffu, size, l);
+                const uint64_t first = __shfl_sync(0xffffffffu, my_first, l);
+                const unsigned cnt = __shfl_sync(0xffffffffu, nch, l);
+                if (first + cnt > a.chunk_cap) continue;
+                for (unsigned c = lane; c < cnt; c += 32) {
+                    uint64_t off, len;
+                    chunk_range(d0, sz, c, off, len);
+                    put_item(a.chunk_q + first + c, s0 + off, d0 + off, len);
+                }
+            }
+        }
+    }
+
+    // ================================================================ grid barrier
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        atomicAdd(&ctl->arrive, 1u);
+        while (ld_acquire_u32(&ctl->arrive) < gridDim.x) {}
+    }
+    __syncthreads();
+    const bool ok = __ldcg(&ctl->bad_inv) == 0;
+    if (blockIdx.x == 0 && tid == 0) ctl->t_mid = globaltimer();
+
+    if (ok) {
+        // ============================================================ counters (a6)
+        if (use_hist) {
+            for (uint32_t s = tid; s < 2 * n_slots; s += kThreads) {
+                const unsigned v = hist[s];
+                if (v) atomicAdd(s < n_slots ? &a.sent[s] : &a.recv[s - n_slots], (unsigned long long)v);
+            }
+        } else {
+            // slot table too large for the shared-memory histogram: count straight into the
+            // cumulative counters, now that the batch is known to be valid
+            for (uint64_t tile = (uint64_t)blockIdx.x * kThreads; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
+                const uint64_t i = tile + tid;
+                uint32_t ss = 0xffffffffu, ds = 0xffffffffu;
+                if (i < a.n) {
+                    const uint4 lo = __ldg(reinterpret_cast<const uint4 *>(a.descs + i));
+                    ds = lo.x;
+                    ss = lo.y;
+                }
+                const unsigned ms = __match_any_sync(0xffffffffu, ss);
+                if (i < a.n && lane == __ffs(ms) - 1) atomicAdd(&a.sent[ss], (unsigned long long)__popc(ms));
+                const unsigned md = __match_any_sync(0xffffffffu, ds);
+                if (i < a.n && lane == __ffs(md) - 1) atomicAdd(&a.recv[ds], (unsigned long long)__popc(md));
+            }
+        }
+
+        // ============================================================ phase B (a4, a5)
+        const unsigned n_chunk = __ldcg(&ctl->n_chunk), n_small = __ldcg(&ctl->n_small);
+        const unsigned n_tickets = n_chunk + (n_small + kWarps - 1) / kWarps;
+        if (tid == 0) sh_ticket[0] = atomicAdd(&ctl->ticket, 1u);
+        __syncthreads();
+        int par = 0;
+        while (true) {
+            const unsigned t = sh_ticket[par];
+            if (t >= n_tickets) break;
+            if (tid == 0) sh_ticket[par ^ 1] = atomicAdd(&ctl->ticket, 1u);   // next round's ticket, a round ahead
+            if (t < n_chunk) {
+                // (a5) the whole CTA copies one chunk
+                const WorkItem w = load_item(a.chunk_q + t);
+                unsigned char *d = reinterpret_cast<unsigned char *>(w.dst);
+                const unsigned char *s = reinterpret_cast<const unsigned char *>(w.src);
+                if (((w.src | w.dst | w.size) & 15) == 0 && w.size >= a.tma_min) {
+                    if (lane == 0) tma_copy_pieces(tma, d, s, w.size, warp, kWarps);
+                    __syncwarp();
+                } else {
+                    copy_span<kUnroll, kLdDefault, uint32_t, kUnrollShifted>(d, s, (uint32_t)w.size, tid, kThreads);
+                }
+            } else {
+                // (a4) one warp per small descriptor
+                const unsigned i = (t - n_chunk) * kWarps + warp;
+                if (i < n_small) {
+                    const WorkItem w = load_item(a.small_q + i);
+                    unsigned char *d = reinterpret_cast<unsigned char *>(w.dst);
+                    const unsigned char *s = reinterpret_cast<const unsigned char *>(w.src);
+                    if (((w.src | w.dst | w.size) & 15) == 0 && w.size >= a.tma_min) {
+                        if (lane == 0) tma_copy_pieces(tma, d, s, w.size, 0, 1);
+                        __syncwarp();
+                    } else {
+                        copy_span<kUnroll, kLdDefault, uint32_t, kUnrollShifted>(d, s, (uint32_t)w.size, lane, 32);
+                    }
+                }
+            }
+            __syncthreads();
+            par ^= 1;
+        }
+        if (lane == 0) tma_drain(tma);
+    }
+
+    // ================================================================ finish (feeds a7)
+    __syncthreads();
+    if (tid == 0) {
+        __threadfence();
+        sh_flag = atomicAdd(&ctl->done, 1u) == gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!sh_flag) return;
+    // last CTA: every CTA's copies and counter updates are complete and visible
+    __threadfence();
+    for (uint32_t s = tid; s < a.n_push; s += kThreads) {
+        a.push[s] = __ldcg(&a.sent[s]);
+        a.push[kPushSlots + s] = __ldcg(&a.recv[s]);
+    }
+    __threadfence_system();
+    __syncthreads();
+    if (tid == 0) {
+        HostRecord *r = a.rec;
+        r->bad_inv = __ldcg(&ctl->bad_inv);
+        r->n_small = __ldcg(&ctl->n_small);
+        r->n_chunk = __ldcg(&ctl->n_chunk);
+        r->t_start = __ldcg(&ctl->t_start);
+        r->t_mid = __ldcg(&ctl->t_mid);
+        r->t_end = globaltimer();
+        // self-clean: the next batch on the stream finds an all-zero control block
+        ctl->bad_inv = 0;
+        ctl->n_small = 0;
+        ctl->n_chunk = 0;
+        ctl->arrive = 0;
+        ctl->ticket = 0;
+        ctl->done = 0;
+        __threadfence_system();
+        *reinterpret_cast<volatile unsigned long long *>(&r->seq) = a.seq;
     }
 }
 
@@ -233,8 +357,9 @@ static int ensure_queues(hicr_ctx *ctx, uint64_t n)
         ctx->small_cap = cap;
     }
     // With pairwise-disjoint destinations (the epoch precondition) a batch expands into
-    // at most n + registered_bytes / kChunkBytes chunks.
-    const uint64_t need = n + ctx->registered_bytes / kChunkBytes + 64;
+    // at most 2 n + registered_bytes / kChunkBytes chunks (a first and a last partial one
+    // per descriptor).
+    const uint64_t need = 2 * n + ctx->registered_bytes / kChunkBytes + 64;
     if (need > ctx->chunk_cap) {
         uint64_t cap = std::max(need, ctx->chunk_cap * 2);
         HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
@@ -268,6 +393,25 @@ static int get_stage(hicr_ctx *ctx, size_t bytes, StageBlock *out)
     return HICR_OK;
 }
 
+size_t engine_smem_bytes(uint32_t n_slots)
+{
+    return (size_t)kWarps * kTmaPiece + (n_slots <= kSmemSlotHist ? 2 * (size_t)n_slots * sizeof(unsigned) : 0);
+}
+
+// Co-resident CTAs of the engine kernel (what a cooperative launch may use).
+int engine_setup(hicr_ctx *ctx)
+{
+    int per_sm = 0;
+    HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, engine_kernel, kThreads,
+                                                                 engine_smem_bytes(kSmemSlotHist)));
+    if (per_sm < 1) return HICR_ERR_NO_CAPACITY;
+    ctx->engine_grid = ctx->num_sms * std::min(per_sm, kCtasPerSm);
+    const char *e = getenv("HICR_TMA_MIN");
+    if (e && *e) ctx->tma_min = (uint32_t)strtoul(e, nullptr, 0);
+    if (ctx->tma_min < 16) ctx->tma_min = 16;
+    return HICR_OK;
+}
+
 }  // namespace hicr
 
 using namespace hicr;
@@ -280,31 +424,30 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     if (n >= (1ull << 32)) return HICR_ERR_NO_CAPACITY;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
 
-    uint64_t n_small_host = n, n_chunk_host = ~0ull;  // upper bounds used to size the grids
+    uint64_t units = ~0ull;   // work tickets of the copy phase, when the host knows them
     const hicr_desc_t *d_descs = descs;
     if (!descs_on_device) {
         // (a2) host-resident table: validate here, all-or-nothing, lowest bad index
         uint64_t ns = 0, nc = 0;
+        const size_t nslots = ctx->slots.size();
+        const SlotRow *rows = ctx->slots.data();
         for (uint64_t i = 0; i < n; i++) {
             const hicr_desc_t &d = descs[i];
             int rc = HICR_OK;
-            if (d.dst_slot >= ctx->slots.size() || ctx->slots[d.dst_slot].size == kInvalidSize)
-                rc = HICR_ERR_INVALID_SLOT;
-            else if (d.dst_off > ctx->slots[d.dst_slot].size || d.size > ctx->slots[d.dst_slot].size - d.dst_off)
+            if (d.dst_slot >= nslots || rows[d.dst_slot].size == kInvalidSize) rc = HICR_ERR_INVALID_SLOT;
+            else if (d.dst_off > rows[d.dst_slot].size || d.size > rows[d.dst_slot].size - d.dst_off)
                 rc = HICR_ERR_OUT_OF_BOUNDS;
-            else if (d.src_slot >= ctx->slots.size() || ctx->slots[d.src_slot].size == kInvalidSize)
-                rc = HICR_ERR_INVALID_SLOT;
-            else if (d.src_off > ctx->slots[d.src_slot].size || d.size > ctx->slots[d.src_slot].size - d.src_off)
+            else if (d.src_slot >= nslots || rows[d.src_slot].size == kInvalidSize) rc = HICR_ERR_INVALID_SLOT;
+            else if (d.src_off > rows[d.src_slot].size || d.size > rows[d.src_slot].size - d.src_off)
                 rc = HICR_ERR_OUT_OF_BOUNDS;
             if (rc != HICR_OK) {
                 if (first_bad) *first_bad = i;
                 return rc;
             }
-            if (d.size > kSmallMax) nc += (d.size + kChunkBytes - 1) / kChunkBytes;
+            if (d.size > kSmallMax) nc += d.size / kChunkBytes + 2;
             else if (d.size) ns++;
         }
-        n_small_host = ns;
-        n_chunk_host = nc;
+        units = nc + (ns + kWarps - 1) / kWarps;
         StageBlock b;
         int rc = get_stage(ctx, n * sizeof(hicr_desc_t), &b);
         if (rc != HICR_OK) return rc;
@@ -314,53 +457,45 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         d_descs = static_cast<const hicr_desc_t *>(b.dev);
     }
 
-    if (ctx->batches_in_epoch == kCtlRing) {
+    if (ctx->batches_in_epoch == kRecRing) {
         int rc = drain_epoch(ctx, false);
         if (rc != HICR_OK) return rc;
     }
     int rc = ensure_queues(ctx, n);
     if (rc != HICR_OK) return rc;
-    if (n_chunk_host != ~0ull && n_chunk_host > ctx->chunk_cap) {
-        // only possible when destinations overlap (precondition violated): refuse cleanly
-        return HICR_ERR_NO_CAPACITY;
-    }
 
-    if (ctx->copy_ctas_per_sm == 0) {
-        int a = 0, b = 0;
-        HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&a, copy_small_kernel, kCopyThreads, 0));
-        HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b, copy_chunk_kernel, kCopyThreads, 0));
-        ctx->copy_ctas_per_sm = std::max(1, std::min(a, b));
-    }
-    const uint32_t n_slots = (uint32_t)ctx->slots.size();
-    Ctl *ctl = ctx->d_ctl + ctx->batches_in_epoch;
-    const unsigned plan_grid = (unsigned)((n + kPlanThreads - 1) / kPlanThreads);
-    const size_t hist_bytes = n_slots <= kSmemSlotHist ? 2 * (size_t)n_slots * sizeof(unsigned) : 0;
-    const unsigned persistent = (unsigned)(ctx->num_sms * ctx->copy_ctas_per_sm);
+    EngineArgs a;
+    a.descs = d_descs;
+    a.n = n;
+    a.slots = ctx->d_slots;
+    a.n_slots = (uint32_t)ctx->slots.size();
+    a.tma_min = ctx->tma_min;
+    a.ctl = ctx->d_ctl;
+    a.small_q = ctx->d_small;
+    a.small_cap = ctx->small_cap;
+    a.chunk_q = ctx->d_chunk;
+    a.chunk_cap = ctx->chunk_cap;
+    a.sent = ctx->d_sent;
+    a.recv = ctx->d_recv;
+    a.rec = ctx->d_rec + ctx->batches_in_epoch;
+    a.push = reinterpret_cast<unsigned long long *>(ctx->d_rec + kRecRing);
+    a.n_push = std::min<uint32_t>(a.n_slots, kPushSlots);
+    a.pad = 0;
+    a.seq = ctx->batch_seq + 1;
 
-    const bool prof = ctx->profiling;
-    if (prof) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
-    plan_kernel<<<plan_grid, kPlanThreads, hist_bytes, ctx->stream>>>(
-        d_descs, n, ctx->d_slots, n_slots, ctl, ctx->d_small, ctx->small_cap, ctx->d_chunk, ctx->chunk_cap,
-        ctx->d_pending, ctx->d_sent, ctx->d_recv);
+    // grid: every co-resident CTA unless the host knows the batch is smaller than that
+    uint64_t want = std::max<uint64_t>((n + kThreads - 1) / kThreads, units == ~0ull ? (uint64_t)ctx->engine_grid : units);
+    const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(want, (uint64_t)ctx->engine_grid));
+    void *args[] = {&a};
+    if (ctx->profiling) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
+    HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args,
+                                               engine_smem_bytes(a.n_slots), ctx->stream));
     ctx->launches++;
-    if (prof) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[1], ctx->stream));
-    if (n_small_host) {
-        const uint64_t want = (n_small_host + kCopyThreads / 32 - 1) / (kCopyThreads / 32);
-        const unsigned grid = (unsigned)std::min<uint64_t>(want, persistent);
-        copy_small_kernel<<<grid, kCopyThreads, 0, ctx->stream>>>(ctl, ctx->d_small);
-        ctx->launches++;
-    }
-    if (prof) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[2], ctx->stream));
-    if (n_chunk_host) {
-        const unsigned grid = (unsigned)std::min<uint64_t>(n_chunk_host, persistent);
-        copy_chunk_kernel<<<grid, kCopyThreads, 0, ctx->stream>>>(ctl, ctx->d_chunk);
-        ctx->launches++;
-    }
-    if (prof) {
-        HICR_CUDA(ctx, cudaEventRecord(ctx->ev[3], ctx->stream));
+    if (ctx->profiling) {
+        HICR_CUDA(ctx, cudaEventRecord(ctx->ev[1], ctx->stream));
         ctx->ev_valid = true;
     }
-    HICR_CUDA(ctx, cudaGetLastError());
+    ctx->batch_seq++;
     ctx->batches_in_epoch++;
     ctx->epoch_open = true;
     return HICR_OK;

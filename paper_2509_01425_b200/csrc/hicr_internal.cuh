@@ -16,14 +16,19 @@ namespace hicr {
 
 // ---------------------------------------------------------------- tunables / classes
 // size <= kSmallMax  : warp-per-descriptor queue (a4)
-// size >  kSmallMax  : split into chunks of kChunkBytes, CTA-per-chunk queue (a5)
+// size >  kSmallMax  : split at kChunkBytes-aligned destination addresses, CTA-per-chunk queue (a5)
 constexpr uint64_t kSmallMax = 8192;
 constexpr uint64_t kChunkBytes = 32768;
-constexpr int kPlanThreads = 256;
-constexpr int kCopyThreads = 256;          // 8 warps per CTA in both copy kernels
-constexpr int kUnroll = 8;                 // 16-byte vectors in flight per lane
-constexpr int kCtlRing = 64;               // control blocks (= batches) per epoch before an internal drain
+constexpr int kThreads = 256;              // 8 warps per CTA of the engine kernel
+constexpr int kWarps = kThreads / 32;
+constexpr int kCtasPerSm = 4;              // persistent grid = SMs x kCtasPerSm (<= 64 registers per thread)
+constexpr int kUnroll = 8;                 // 16-byte vectors in flight per lane (aligned source)
+constexpr int kUnrollShifted = 4;          // the same for byte-shifted sources (keeps the kernel at 64 registers)
 constexpr uint32_t kSmemSlotHist = 1024;   // per-CTA shared-memory counter histogram up to this many slots
+constexpr uint32_t kTmaPiece = 4096;       // bytes per bulk copy; one shared-memory stage per warp
+constexpr uint32_t kTmaMinDefault = 1024;  // aligned spans of at least this many bytes take the TMA bulk path
+constexpr int kRecRing = 64;               // host completion records (= batches per epoch before an internal drain)
+constexpr uint32_t kPushSlots = 256;       // counters of the first kPushSlots slots are pushed into the record area
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
 constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3;
@@ -44,16 +49,32 @@ struct __align__(16) WorkItem {
     uint64_t pad;
 };
 
-// Per-batch control block, reset to all-zero by one memset at the fence.
-struct __align__(64) Ctl {
-    unsigned long long bad_inv;  // atomicMax of ~((index << 4) | error id); 0 = no error
-    unsigned int n_small;        // items in the warp queue
-    unsigned int n_chunk;        // items in the CTA queue
-    unsigned int done;           // plan-kernel CTA ticket
-    unsigned int go;             // 1 = validated and committed: copy kernels may run
-    unsigned int pad[10];
+// Device control block of the engine kernel.  All-zero between batches: the last CTA of
+// a batch publishes the host record and then clears it, so consecutive batches on the
+// stream reuse it without any memset.
+struct __align__(128) Ctl {
+    unsigned long long bad_inv;   // atomicMax of ~((index << 4) | error id); 0 = no error
+    unsigned long long t_start;   // %globaltimer at kernel start (CTA 0)
+    unsigned long long t_mid;     // %globaltimer after the grid barrier (CTA 0)
+    unsigned int n_small;         // items in the warp queue
+    unsigned int n_chunk;         // items in the CTA queue
+    unsigned int arrive;          // grid barrier between validation/binning and the copies
+    unsigned int ticket;          // dynamic work tickets of the copy phase
+    unsigned int done;            // CTAs that finished the copy phase
+    unsigned int pad[21];
 };
-static_assert(sizeof(Ctl) == 64, "Ctl is one 64-byte block");
+static_assert(sizeof(Ctl) == 128, "Ctl is one 128-byte line");
+
+// Completion record of one batch, written by the last CTA into mapped pinned host memory;
+// `seq` is written last (after a system-scope fence) and is what hicr_fence polls.
+struct __align__(64) HostRecord {
+    unsigned long long seq;
+    unsigned long long bad_inv;
+    unsigned long long t_start, t_mid, t_end;
+    unsigned int n_small, n_chunk;
+    unsigned long long pad[2];
+};
+static_assert(sizeof(HostRecord) == 64, "HostRecord is 64 bytes");
 
 // Channel state in device memory; head and tail on separate 128 B lines so the
 // producer's and the consumer's polls do not share a line.
@@ -73,51 +94,55 @@ struct CallResult {
 
 #ifdef __CUDACC__
 // ---------------------------------------------------------------- device helpers
-enum LdPolicy { kLdStream = 0, kLdL2 = 1 };
+enum LdPolicy { kLdStream = 0, kLdL2 = 1, kLdDefault = 2 };
 
 template <int POL>
 __device__ __forceinline__ uint4 ld16(const uint4 *p)
 {
-    return POL == kLdStream ? __ldcs(p) : __ldcg(p);
+    return POL == kLdStream ? __ldcs(p) : POL == kLdL2 ? __ldcg(p) : *p;
 }
 template <int POL>
 __device__ __forceinline__ unsigned char ld1(const unsigned char *p)
 {
-    return POL == kLdStream ? __ldcs(p) : __ldcg(p);
+    return POL == kLdStream ? __ldcs(p) : POL == kLdL2 ? __ldcg(p) : *p;
 }
 template <int POL>
 __device__ __forceinline__ void st16(uint4 *p, uint4 v)
 {
-    if (POL == kLdStream) __stcs(p, v); else __stcg(p, v);
+    if (POL == kLdStream) __stcs(p, v); else if (POL == kLdL2) __stcg(p, v); else *p = v;
 }
 
-// dst vector = 16 bytes starting `shift` = 4*Q + r bytes into the 32-byte pair (a, nx).
-template <int Q>
-__device__ __forceinline__ uint4 shift_combine(const uint4 &a, const uint4 &nx, unsigned rbits)
+// dst vector = 16 bytes starting 4*q + rbits/8 bytes into the 32-byte pair (a, nx); q in 0..3.
+__device__ __forceinline__ uint4 shift_combine(const uint4 &a, const uint4 &nx, unsigned q, unsigned rbits)
 {
-    const unsigned w[8] = {a.x, a.y, a.z, a.w, nx.x, nx.y, nx.z, nx.w};
+    // five consecutive words starting at word q of {a.x a.y a.z a.w nx.x nx.y nx.z nx.w}
+    const bool q1 = q & 1, q2 = q & 2;
+    const unsigned e0 = q1 ? a.y : a.x, e1 = q1 ? a.z : a.y, e2 = q1 ? a.w : a.z, e3 = q1 ? nx.x : a.w,
+                   e4 = q1 ? nx.y : nx.x, e5 = q1 ? nx.z : nx.y, e6 = q1 ? nx.w : nx.z;
+    const unsigned w0 = q2 ? e2 : e0, w1 = q2 ? e3 : e1, w2 = q2 ? e4 : e2, w3 = q2 ? e5 : e3, w4 = q2 ? e6 : e4;
     uint4 o;
-    o.x = __funnelshift_r(w[Q + 0], w[Q + 1], rbits);
-    o.y = __funnelshift_r(w[Q + 1], w[Q + 2], rbits);
-    o.z = __funnelshift_r(w[Q + 2], w[Q + 3], rbits);
-    o.w = __funnelshift_r(w[Q + 3], w[Q + 4], rbits);
+    o.x = __funnelshift_r(w0, w1, rbits);
+    o.y = __funnelshift_r(w1, w2, rbits);
+    o.z = __funnelshift_r(w2, w3, rbits);
+    o.w = __funnelshift_r(w3, w4, rbits);
     return o;
 }
 
-// Body of a copy whose destination is 16 B-aligned and whose source is `4*Q + r` bytes
+// Body of a copy whose destination is 16 B-aligned and whose source is `4*q + rbits/8` bytes
 // past a 16 B boundary (not both zero).  sA = source rounded down to 16 B.  Each warp
 // takes tiles of 32*U consecutive destination vectors; lane l loads aligned source
 // vectors l, l+32, ... once, and gets the vector after its own from lane l+1 by shuffle
 // (lane 31 from lane 0's next load), so every source byte is requested from L2 once.
-template <int U, int POL, int Q>
+template <int U, int POL, typename IDX>
 __device__ __forceinline__ void copy_body_shifted(uint4 *__restrict__ d4, const uint4 *__restrict__ sA,
-                                                  uint64_t nvec, unsigned rbits, int lane, int warp, int nwarps)
+                                                  IDX nvec, unsigned q, unsigned rbits, int lane, int warp,
+                                                  int nwarps)
 {
-    constexpr uint64_t kTile = 32ull * U;
-    const uint64_t nfull = nvec / kTile;
+    constexpr IDX kTile = 32 * U;
+    const IDX nfull = nvec / kTile;
     const int nxt_lane = (lane + 1) & 31;
-    for (uint64_t t = warp; t < nfull; t += nwarps) {
-        const uint64_t base = t * kTile + lane;
+    for (IDX t = warp; t < nfull; t += nwarps) {
+        const IDX base = t * kTile + lane;
         uint4 a[U + 1];
 #pragma unroll
         for (int u = 0; u < U; u++) a[u] = ld16<POL>(sA + base + 32 * u);
@@ -131,14 +156,14 @@ __device__ __forceinline__ void copy_body_shifted(uint4 *__restrict__ d4, const 
             nx.y = __shfl_sync(0xffffffffu, give.y, nxt_lane);
             nx.z = __shfl_sync(0xffffffffu, give.z, nxt_lane);
             nx.w = __shfl_sync(0xffffffffu, give.w, nxt_lane);
-            st16<POL>(d4 + base + 32 * u, shift_combine<Q>(a[u], nx, rbits));
+            st16<POL>(d4 + base + 32 * u, shift_combine(a[u], nx, q, rbits));
         }
     }
-    const uint64_t rem0 = nfull * kTile;
-    if (rem0 < nvec && warp == (int)(nfull % (uint64_t)nwarps)) {
+    const IDX rem0 = nfull * kTile;
+    if (rem0 < nvec && warp == (int)(nfull % (IDX)nwarps)) {
         // ragged last tile: vector v is stored if v < nvec; aligned source vector v is
         // loaded if v <= nvec (vector nvec still holds bytes of destination vector nvec-1)
-        const uint64_t base = rem0 + lane;
+        const IDX base = rem0 + lane;
         uint4 a[U + 1];
 #pragma unroll
         for (int u = 0; u < U; u++) {
@@ -154,32 +179,34 @@ __device__ __forceinline__ void copy_body_shifted(uint4 *__restrict__ d4, const 
             nx.y = __shfl_sync(0xffffffffu, give.y, nxt_lane);
             nx.z = __shfl_sync(0xffffffffu, give.z, nxt_lane);
             nx.w = __shfl_sync(0xffffffffu, give.w, nxt_lane);
-            if (base + 32 * u < nvec) st16<POL>(d4 + base + 32 * u, shift_combine<Q>(a[u], nx, rbits));
+            if (base + 32 * u < nvec) st16<POL>(d4 + base + 32 * u, shift_combine(a[u], nx, q, rbits));
         }
     }
 }
 
-template <int U, int POL>
+template <int U, int POL, typename IDX>
 __device__ __forceinline__ void copy_body_aligned(uint4 *__restrict__ d4, const uint4 *__restrict__ s4,
-                                                  uint64_t nvec, int lane, int warp, int nwarps)
+                                                  IDX nvec, int lane, int warp, int nwarps)
 {
-    constexpr uint64_t kTile = 32ull * U;
-    const uint64_t nfull = nvec / kTile;
-    for (uint64_t t = warp; t < nfull; t += nwarps) {
-        const uint64_t base = t * kTile + lane;
+    constexpr IDX kTile = 32 * U;
+    const IDX nfull = nvec / kTile;
+    for (IDX t = warp; t < nfull; t += nwarps) {
+        const IDX base = t * kTile + lane;
         uint4 a[U];
 #pragma unroll
         for (int u = 0; u < U; u++) a[u] = ld16<POL>(s4 + base + 32 * u);
 #pragma unroll
         for (int u = 0; u < U; u++) st16<POL>(d4 + base + 32 * u, a[u]);
     }
-    const uint64_t rem0 = nfull * kTile;
-    if (rem0 < nvec && warp == (int)(nfull % (uint64_t)nwarps)) {
-        const uint64_t base = rem0 + lane;
+    const IDX rem0 = nfull * kTile;
+    if (rem0 < nvec && warp == (int)(nfull % (IDX)nwarps)) {
+        const IDX base = rem0 + lane;
         uint4 a[U];
 #pragma unroll
-        for (int u = 0; u < U; u++)
+        for (int u = 0; u < U; u++) {
+            a[u] = make_uint4(0, 0, 0, 0);
             if (base + 32 * u < nvec) a[u] = ld16<POL>(s4 + base + 32 * u);
+        }
 #pragma unroll
         for (int u = 0; u < U; u++)
             if (base + 32 * u < nvec) st16<POL>(d4 + base + 32 * u, a[u]);
@@ -190,38 +217,34 @@ __device__ __forceinline__ void copy_body_aligned(uint4 *__restrict__ d4, const 
 // group of `gsize` threads (a multiple of 32: one warp, or a whole CTA), gtid in
 // [0, gsize).  Byte head up to the first 16 B boundary of dst, 16 B vector body with
 // aligned stores (aligned or byte-shifted loads), byte tail (a4/a5 of SURVEY.md S8(a)).
-template <int U, int POL>
+// IDX = uint32_t when n < 2^32 is known (fewer registers).  U / US = 16 B vectors in flight per
+// lane in the aligned / byte-shifted body.
+template <int U, int POL, typename IDX = uint64_t, int US = U>
 __device__ __forceinline__ void copy_span(unsigned char *__restrict__ dst, const unsigned char *__restrict__ src,
-                                          uint64_t n, int gtid, int gsize)
+                                          IDX n, int gtid, int gsize)
 {
     const int lane = gtid & 31, warp = gtid >> 5, nwarps = gsize >> 5;
-    uint64_t head = (16 - (reinterpret_cast<uintptr_t>(dst) & 15)) & 15;
+    IDX head = (IDX)((16 - (reinterpret_cast<uintptr_t>(dst) & 15)) & 15);
     if (head > n) head = n;
-    if ((uint64_t)gtid < head) dst[gtid] = ld1<POL>(src + gtid);
+    if ((IDX)gtid < head) dst[gtid] = ld1<POL>(src + gtid);
     dst += head;
     src += head;
     n -= head;
-    const uint64_t nvec = n >> 4;
+    const IDX nvec = n >> 4;
     const unsigned tail = (unsigned)(n & 15);
     {
         const unsigned t = (unsigned)(gsize - 1 - gtid);   // the last threads take the tail
-        if (t < tail) dst[nvec * 16 + t] = ld1<POL>(src + nvec * 16 + t);
+        if (t < tail) dst[(size_t)nvec * 16 + t] = ld1<POL>(src + (size_t)nvec * 16 + t);
     }
     if (nvec == 0) return;
     uint4 *d4 = reinterpret_cast<uint4 *>(dst);
     const unsigned s = (unsigned)(reinterpret_cast<uintptr_t>(src) & 15);
     if (s == 0) {
-        copy_body_aligned<U, POL>(d4, reinterpret_cast<const uint4 *>(src), nvec, lane, warp, nwarps);
+        copy_body_aligned<U, POL, IDX>(d4, reinterpret_cast<const uint4 *>(src), nvec, lane, warp, nwarps);
         return;
     }
     const uint4 *sA = reinterpret_cast<const uint4 *>(src - s);
-    const unsigned rbits = (s & 3) * 8;
-    switch (s >> 2) {
-    case 0: copy_body_shifted<U, POL, 0>(d4, sA, nvec, rbits, lane, warp, nwarps); break;
-    case 1: copy_body_shifted<U, POL, 1>(d4, sA, nvec, rbits, lane, warp, nwarps); break;
-    case 2: copy_body_shifted<U, POL, 2>(d4, sA, nvec, rbits, lane, warp, nwarps); break;
-    default: copy_body_shifted<U, POL, 3>(d4, sA, nvec, rbits, lane, warp, nwarps); break;
-    }
+    copy_body_shifted<US, POL, IDX>(d4, sA, nvec, s >> 2, (s & 3) * 8, lane, warp, nwarps);
 }
 
 __device__ __forceinline__ unsigned long long ld_acquire(const unsigned long long *p)
@@ -234,6 +257,83 @@ __device__ __forceinline__ void st_release(unsigned long long *p, unsigned long 
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
+
+// ---- 1-D bulk async copies (TMA) through shared memory, completion by mbarrier transaction
+// bytes on the way in and by bulk async-groups on the way out.  Addresses and sizes must
+// be multiples of 16 bytes.
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(uint64_t *bar, unsigned count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, unsigned bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, unsigned parity)
+{
+    unsigned ok = 0;
+    while (!ok) {
+        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}\n"
+                     : "=r"(ok)
+                     : "r"(smem_u32(bar)), "r"(parity)
+                     : "memory");
+    }
+}
+__device__ __forceinline__ void bulk_g2s(void *smem_dst, const void *gsrc, unsigned bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                     smem_u32(smem_dst)),
+                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_s2g(void *gdst, const void *smem_src, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gdst), "r"(smem_u32(smem_src)),
+                 "r"(bytes)
+                 : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
+
+// State of one warp's bulk-copy driver (lane 0): one kTmaPiece stage and its mbarrier.
+struct TmaLane {
+    unsigned char *stage;
+    uint64_t *bar;
+    unsigned phase;     // parity of the next mbarrier completion
+    bool pending;       // a bulk store may still be reading the stage
+};
+
+// Driver lane only: dst[0, n) = src[0, n) for piece indices first, first + stride, ... of
+// kTmaPiece bytes each; dst, src and n are multiples of 16.  Global -> shared (mbarrier
+// complete_tx), then shared -> global (bulk group); the stage is reused once the store has
+// finished READING it, the writes are completed by tma_drain() before the CTA signals done.
+__device__ __forceinline__ void tma_copy_pieces(TmaLane &t, unsigned char *dst, const unsigned char *src, uint64_t n,
+                                                unsigned first, unsigned stride)
+{
+    for (uint64_t off = (uint64_t)first * kTmaPiece; off < n; off += (uint64_t)stride * kTmaPiece) {
+        const unsigned len = (unsigned)min((uint64_t)kTmaPiece, n - off);
+        if (t.pending) bulk_wait_read_all();
+        mbar_expect_tx(t.bar, len);
+        bulk_g2s(t.stage, src + off, len, t.bar);
+        mbar_wait(t.bar, t.phase);
+        t.phase ^= 1;
+        bulk_s2g(dst + off, t.stage, len);
+        bulk_commit();
+        t.pending = true;
+    }
+}
+__device__ __forceinline__ void tma_drain(TmaLane &t)
+{
+    if (t.pending) {
+        bulk_wait_all();       // the bulk stores are complete, not only done reading shared memory
+        fence_proxy_async();   // order the async-proxy writes before the generic-proxy release below
+        t.pending = false;
+    }
+}
+
 #endif  // __CUDACC__
 
 // ---------------------------------------------------------------- host-side context
@@ -258,12 +358,15 @@ struct hicr_ctx {
     hicr::SlotRow *d_slots = nullptr;        // [HICR_MAX_SLOTS]
     unsigned long long *d_sent = nullptr;    // [HICR_MAX_SLOTS]
     unsigned long long *d_recv = nullptr;    // [HICR_MAX_SLOTS]
-    unsigned int *d_pending = nullptr;       // [2 * HICR_MAX_SLOTS] per-batch counts before commit
     uint64_t registered_bytes = 0;
 
-    // per-batch control blocks of the current epoch
-    hicr::Ctl *d_ctl = nullptr;              // [kCtlRing]
-    uint32_t batches_in_epoch = 0;           // since the last fence (or internal drain)
+    // engine control block (device, self-cleaning) and per-batch completion records
+    // (mapped pinned host memory: kRecRing records, then 2 * kPushSlots pushed counters)
+    hicr::Ctl *d_ctl = nullptr;
+    hicr::HostRecord *h_rec = nullptr;       // host view
+    hicr::HostRecord *d_rec = nullptr;       // device alias
+    uint64_t batch_seq = 0;                  // sequence number of the last launched batch (1-based)
+    uint32_t batches_in_epoch = 0;           // records in use since the last fence (or internal drain)
     uint64_t epoch_batch_base = 0;           // batches drained earlier in this epoch
     bool epoch_open = false;                 // any work enqueued since the last fence
     int epoch_error = HICR_OK;               // first deferred error found so far in this epoch
@@ -280,7 +383,7 @@ struct hicr_ctx {
     // staging of host-resident descriptor tables (returned to `free_stage` at the fence)
     std::vector<hicr::StageBlock> free_stage, used_stage;
 
-    // fence read-back (pinned)
+    // counter read-back for slot tables larger than kPushSlots (pinned)
     unsigned char *h_fence = nullptr;
     size_t h_fence_bytes = 0;
 
@@ -289,17 +392,20 @@ struct hicr_ctx {
     hicr::CallResult *d_call = nullptr;      // device alias of h_call
 
     uint64_t launches = 0;
-    int copy_ctas_per_sm = 0;
+    int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
+    uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
 
     bool profiling = false;
-    cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+    cudaEvent_t ev[2] = {nullptr, nullptr};
     bool ev_valid = false;
+    hicr::HostRecord last_rec = {};          // record of the last completed batch (profile_read)
 };
 
 namespace hicr {
 int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what);
 int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
+int engine_setup(hicr_ctx *ctx);
 }  // namespace hicr
 
 #define HICR_CUDA(ctx, call)                                                   \
