@@ -7,6 +7,7 @@
 #include "hicr_internal.cuh"
 
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 
 namespace hicr {
@@ -45,44 +46,63 @@ int refresh_counters(hicr_ctx *ctx)
     return HICR_OK;
 }
 
-// Wait until the engine kernel of batch `seq` has published its completion record `r`
-// (mapped pinned memory).  Polls the record; every so often asks the stream, so that a
-// faulted kernel turns into HICR_ERR_CUDA instead of a hang.
-static int wait_record(hicr_ctx *ctx, const HostRecord *r, uint64_t seq)
+// One flagged word of a completion record (see HostRecord): true once it carries `flag`.
+static inline bool word_ready(const unsigned long long *w, uint32_t flag, uint32_t *payload)
 {
-    const volatile unsigned long long *flag = &r->seq;
-    for (unsigned spins = 0;; spins++) {
-        if (*flag == seq) break;
-        if ((spins & 0x3fff) == 0x3fff) {
-            cudaError_t e = cudaStreamQuery(ctx->stream);
-            if (e == cudaSuccess) {
-                if (*flag == seq) break;
-                ctx->cuda_error = "engine kernel finished without publishing its completion record";
-                return HICR_ERR_CUDA;
+    const unsigned long long v = *reinterpret_cast<const volatile unsigned long long *>(w);
+    if ((uint32_t)(v >> 32) != flag) return false;
+    *payload = (uint32_t)v;
+    return true;
+}
+
+// Wait until `n` flagged words starting at `w` all carry `flag`; payloads go to out[].
+// Polls; every so often asks the stream, so that a faulted kernel turns into HICR_ERR_CUDA
+// instead of a hang.
+static int wait_words(hicr_ctx *ctx, const unsigned long long *w, size_t n, uint32_t flag, uint32_t *out)
+{
+    unsigned spins = 0;
+    for (size_t i = 0; i < n; i++) {
+        while (!word_ready(w + i, flag, out + i)) {
+            if ((++spins & 0x3fff) == 0) {
+                cudaError_t e = cudaStreamQuery(ctx->stream);
+                if (e == cudaSuccess) {
+                    if (word_ready(w + i, flag, out + i)) break;
+                    ctx->cuda_error = "engine kernel finished without publishing its completion record";
+                    return HICR_ERR_CUDA;
+                }
+                if (e != cudaErrorNotReady) return cuda_fail(ctx, e, "cudaStreamQuery(fence)");
             }
-            if (e != cudaErrorNotReady) return cuda_fail(ctx, e, "cudaStreamQuery(fence)");
         }
     }
-    __atomic_thread_fence(__ATOMIC_ACQUIRE);
     return HICR_OK;
 }
 
-// Complete everything enqueued so far in this epoch: wait for the last batch's completion
-// record (stream order makes the earlier ones complete too), fold deferred errors into the
-// epoch state, take the pushed counters and recycle staging.  final_fence distinguishes
-// hicr_fence from the internal drain that happens when an epoch issues more than kRecRing
-// batches.
+static inline uint64_t join64(uint32_t lo, uint32_t hi) { return (uint64_t)lo | ((uint64_t)hi << 32); }
+
+// Complete everything enqueued so far in this epoch: wait for every batch's completion
+// record (the last one first: stream order makes the earlier ones complete too), fold
+// deferred errors into the epoch state, take the pushed counters and recycle staging.
+// final_fence distinguishes hicr_fence from the internal drain that happens when an epoch
+// issues more than kRecRing batches.
 int drain_epoch(hicr_ctx *ctx, bool final_fence)
 {
     const uint32_t nb = ctx->batches_in_epoch;
     const size_t n = ctx->slots.size();
-    if (nb) {
-        int rc = wait_record(ctx, ctx->h_rec + (nb - 1), ctx->batch_seq);
+    uint32_t words[kRwUsed];
+    for (uint32_t k = 0; k < nb; k++) {
+        const uint32_t b = k == 0 ? nb - 1 : k - 1;   // last batch first, then 0 .. nb-2
+        const uint64_t seq = ctx->batch_seq - (nb - 1 - b);
+        int rc = wait_words(ctx, ctx->h_rec[b].w, kRwUsed, rec_flag(seq), words);
         if (rc != HICR_OK) return rc;
-        ctx->last_rec = ctx->h_rec[nb - 1];
+        if (b == nb - 1) {
+            ctx->last_t[0] = join64(words[kRwTStartLo], words[kRwTStartHi]);
+            ctx->last_t[1] = join64(words[kRwTMidLo], words[kRwTMidHi]);
+            ctx->last_t[2] = join64(words[kRwTEndLo], words[kRwTEndHi]);
+        }
+        ctx->rec_bad[b] = join64(words[kRwBadLo], words[kRwBadHi]);
     }
     for (uint32_t b = 0; b < nb; b++) {
-        const unsigned long long bad_inv = ctx->h_rec[b].bad_inv;
+        const unsigned long long bad_inv = ctx->rec_bad[b];
         if (bad_inv != 0 && ctx->epoch_error == HICR_OK) {
             const unsigned long long packed = ~bad_inv;
             ctx->epoch_error = bad_to_status((unsigned)(packed & 15));
@@ -95,9 +115,14 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence)
     if (n && final_fence) {
         if (nb && n <= kPushSlots) {
             // the last batch pushed the cumulative counters next to the records
-            const unsigned long long *push = reinterpret_cast<const unsigned long long *>(ctx->h_rec + kRecRing);
-            memcpy(ctx->sent.data(), push, n * 8);
-            memcpy(ctx->recv.data(), push + kPushSlots, n * 8);
+            int rc = wait_words(ctx, ctx->h_rec[kRecRing].w, n * kPushWordsPerSlot, rec_flag(ctx->batch_seq),
+                                ctx->push_words.data());
+            if (rc != HICR_OK) return rc;
+            for (size_t s = 0; s < n; s++) {
+                const uint32_t *w = ctx->push_words.data() + s * kPushWordsPerSlot;
+                ctx->sent[s] = join64(w[0], w[1]);
+                ctx->recv[s] = join64(w[2], w[3]);
+            }
         } else {
             int rc = refresh_counters(ctx);
             if (rc != HICR_OK) return rc;
@@ -166,7 +191,8 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
     INIT_CUDA(cudaMalloc(&ctx->d_ctl, sizeof(Ctl)));
     INIT_CUDA(cudaMemset(ctx->d_ctl, 0, sizeof(Ctl)));
     {
-        const size_t rec_bytes = sizeof(HostRecord) * kRecRing + 2 * 8 * (size_t)kPushSlots;
+        // kRecRing records, then the pushed counter words (addressed as h_rec[kRecRing].w[...])
+        const size_t rec_bytes = sizeof(HostRecord) * kRecRing + 8 * (size_t)kPushWordsPerSlot * kPushSlots;
         INIT_CUDA(cudaHostAlloc(&ctx->h_rec, rec_bytes, cudaHostAllocMapped));
         memset(ctx->h_rec, 0, rec_bytes);
         INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_rec, ctx->h_rec, 0));
@@ -195,11 +221,13 @@ int hicr_finalize(hicr_ctx_t *ctx)
     if (!ctx) return HICR_ERR_INVALID_ARG;
     (void)cudaSetDevice(ctx->device);
     (void)cudaStreamSynchronize(ctx->stream);
+#ifdef HICR_TRACE
+    if (getenv("HICR_TRACE_FILE")) trace_dump(getenv("HICR_TRACE_FILE"));
+#endif
     cudaFree(ctx->d_slots);
     cudaFree(ctx->d_sent);
     cudaFree(ctx->d_recv);
     cudaFree(ctx->d_ctl);
-    cudaFree(ctx->d_small);
     cudaFree(ctx->d_chunk);
     for (auto *v : {&ctx->free_stage, &ctx->used_stage})
         for (auto &b : *v) {
@@ -316,10 +344,10 @@ int hicr_profile_read(hicr_ctx_t *ctx, float *ms)
 {
     if (!ctx || !ms) return HICR_ERR_INVALID_ARG;
     if (!ctx->ev_valid || ctx->epoch_open) return HICR_ERR_INVALID_ARG;   // only after a fence
-    const HostRecord &r = ctx->last_rec;
-    ms[0] = (float)((double)(r.t_mid - r.t_start) * 1e-6);
-    ms[1] = (float)((double)(r.t_end - r.t_mid) * 1e-6);
-    ms[2] = (float)((double)(r.t_end - r.t_start) * 1e-6);
+    const uint64_t *t = ctx->last_t;
+    ms[0] = (float)((double)(t[1] - t[0]) * 1e-6);
+    ms[1] = (float)((double)(t[2] - t[1]) * 1e-6);
+    ms[2] = (float)((double)(t[2] - t[0]) * 1e-6);
     HICR_CUDA(ctx, cudaEventSynchronize(ctx->ev[1]));
     HICR_CUDA(ctx, cudaEventElapsedTime(&ms[3], ctx->ev[0], ctx->ev[1]));
     return HICR_OK;

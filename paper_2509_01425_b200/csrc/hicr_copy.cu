@@ -27,6 +27,7 @@
 #include "hicr_internal.cuh"
 
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 
@@ -43,6 +44,26 @@ __device__ __forceinline__ unsigned long long globaltimer()
     asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
     return t;
 }
+
+#ifdef HICR_TRACE
+// debug build only (_work probes): per-CTA %globaltimer stamps of the last batch
+__device__ unsigned long long g_trace[8 * 1024];
+#define TRACE(k) do { if (tid == 0 && blockIdx.x < 1024) g_trace[blockIdx.x * 8 + (k)] = globaltimer(); } while (0)
+void trace_dump(const char *path)
+{
+    static unsigned long long h[8 * 1024];
+    if (cudaMemcpyFromSymbol(h, g_trace, sizeof(h)) != cudaSuccess) return;
+    FILE *f = fopen(path, "w");
+    if (!f) return;
+    for (int b = 0; b < 1024; b++) {
+        if (!h[b * 8]) continue;
+        for (int k = 0; k < 8; k++) fprintf(f, "%llu%c", h[b * 8 + k], k == 7 ? '\n' : ' ');
+    }
+    fclose(f);
+}
+#else
+#define TRACE(k) do { } while (0)
+#endif
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
 {
@@ -101,75 +122,137 @@ struct EngineArgs {
     uint32_t n_slots;
     uint32_t tma_min;
     Ctl *ctl;
-    WorkItem *small_q;
-    uint64_t small_cap;
     WorkItem *chunk_q;
     uint64_t chunk_cap;
     unsigned long long *sent;
     unsigned long long *recv;
-    HostRecord *rec;                 // this batch's record (device alias of mapped pinned memory)
-    unsigned long long *push;        // [2 * kPushSlots] pushed counters (device alias of mapped pinned memory)
+    unsigned long long *rec;         // this batch's record words (device alias of mapped pinned memory)
+    unsigned long long *push;        // [kPushWordsPerSlot * kPushSlots] pushed counter words (mapped pinned memory)
     uint32_t n_push;
-    uint32_t pad;
-    unsigned long long seq;
+    uint32_t flag;                   // rec_flag(sequence number of this batch)
+    uint32_t gss;                    // guided self-scheduling divisor: ticket = left / (gss x warps)
+    uint32_t max_group;              // descriptors per warp ticket, at most (<= kMaxGroup)
 };
+
+// One 8-byte word of the completion record: payload in the low half, flag in the high half.
+__device__ __forceinline__ void put_word(unsigned long long *w, uint32_t payload, uint32_t flag)
+{
+    *reinterpret_cast<volatile unsigned long long *>(w) = ((unsigned long long)flag << 32) | payload;
+}
+
+// Slot row `s` (s < n_slots): from the shared-memory cache when the table fits, else from L2.
+__device__ __forceinline__ SlotRow slot_row(const SlotRow *cache, const SlotRow *global, uint32_t n_slots, uint32_t s)
+{
+    if (n_slots <= kSlotCache) return cache[s];
+    const uint4 v = __ldg(reinterpret_cast<const uint4 *>(global + s));
+    SlotRow r;
+    r.base = (uint64_t)v.x | ((uint64_t)v.y << 32);
+    r.size = (uint64_t)v.z | ((uint64_t)v.w << 32);
+    return r;
+}
+
+// The 32 bytes of one descriptor, issued now and consumed later (volatile: the loads stay
+// where they are written, ahead of the copy they overlap with).
+__device__ __forceinline__ void load_desc_raw(const hicr_desc_t *d, uint4 &lo, uint4 &hi)
+{
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];" : "=r"(lo.x), "=r"(lo.y), "=r"(lo.z), "=r"(lo.w) : "l"(d));
+    asm volatile("ld.global.nc.v4.u32 {%0, %1, %2, %3}, [%4];"
+                 : "=r"(hi.x), "=r"(hi.y), "=r"(hi.z), "=r"(hi.w)
+                 : "l"(reinterpret_cast<const unsigned char *>(d) + 16));
+}
+
+// Check one descriptor (its 32 bytes in lo, hi) against the slot table: destination before source,
+// overflow-safe "off + size <= slot size".  Returns 0 or the error id; on success src/dst
+// are absolute addresses.
+__device__ __forceinline__ unsigned resolve(const uint4 &lo, const uint4 &hi, const SlotRow *cache,
+                                            const SlotRow *global, uint32_t n_slots, uint32_t &ds, uint32_t &ss,
+                                            uint64_t &dst, uint64_t &src, uint64_t &size)
+{
+    ds = lo.x;
+    ss = lo.y;
+    const uint64_t dst_off = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
+    const uint64_t src_off = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
+    size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
+    SlotRow dr{0, kInvalidSize}, sr{0, kInvalidSize};
+    if (ds < n_slots) dr = slot_row(cache, global, n_slots, ds);
+    if (ss < n_slots) sr = slot_row(cache, global, n_slots, ss);
+    if (dr.size == kInvalidSize) return kBadInvalidSlot;
+    if (dst_off > dr.size || size > dr.size - dst_off) return kBadOutOfBounds;
+    if (sr.size == kInvalidSize) return kBadInvalidSlot;
+    if (src_off > sr.size || size > sr.size - src_off) return kBadOutOfBounds;
+    dst = dr.base + dst_off;
+    src = sr.base + src_off;
+    return 0;
+}
+
+// A descriptor of a batch already known to be valid: absolute addresses, and its size if it
+// belongs to the warp-per-descriptor class (0 < size <= kSmallMax), else 0.
+__device__ __forceinline__ unsigned resolve_small(const uint4 &lo, const uint4 &hi, const SlotRow *cache,
+                                                  const SlotRow *global, uint32_t n_slots, uint64_t &dst, uint64_t &src)
+{
+    const uint64_t size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
+    if (size == 0 || size > kSmallMax) return 0;
+    dst = slot_row(cache, global, n_slots, lo.x).base + ((uint64_t)lo.z | ((uint64_t)lo.w << 32));
+    src = slot_row(cache, global, n_slots, lo.y).base + ((uint64_t)hi.x | ((uint64_t)hi.y << 32));
+    return (unsigned)size;
+}
+
+// Shared-memory layout of the engine kernel (dynamic): TMA stages, slot cache, histogram.
+constexpr size_t kSmemStages = (size_t)kWarps * kTmaStages * kTmaPiece;
+constexpr size_t kSmemCache = (size_t)kSlotCache * sizeof(SlotRow);
 
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const EngineArgs a)
 {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];   // [kWarps x kTmaPiece stages][histogram]
-    __shared__ uint64_t bars[kWarps];
+    extern __shared__ __align__(128) unsigned char dyn_smem[];   // [stages][slot cache][histogram]
+    __shared__ uint64_t bars[kWarps * kTmaStages];
     __shared__ unsigned sh_ticket[2];
     __shared__ unsigned sh_flag;
-    unsigned int *hist = reinterpret_cast<unsigned int *>(dyn_smem + (size_t)kWarps * kTmaPiece);
+    SlotRow *cache = reinterpret_cast<SlotRow *>(dyn_smem + kSmemStages);
+    unsigned int *hist = reinterpret_cast<unsigned int *>(dyn_smem + kSmemStages + kSmemCache);
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     Ctl *ctl = a.ctl;
     const uint32_t n_slots = a.n_slots;
     const bool use_hist = n_slots <= kSmemSlotHist;
     if (blockIdx.x == 0 && tid == 0) ctl->t_start = globaltimer();
+    TRACE(0);
+    // the first tile's descriptors are requested before anything else, so that their DRAM
+    // round trip overlaps the slot-table fetch and the shared-memory set-up
+    uint4 alo = make_uint4(0, 0, 0, 0), ahi = alo;
+    const uint64_t tile0 = (uint64_t)blockIdx.x * kThreads;
+    if (tile0 + tid < a.n) load_desc_raw(a.descs + tile0 + tid, alo, ahi);
+    if (n_slots <= kSlotCache)
+        for (uint32_t i = tid; i < n_slots; i += kThreads) {
+            const uint4 v = __ldg(reinterpret_cast<const uint4 *>(a.slots + i));
+            cache[i].base = (uint64_t)v.x | ((uint64_t)v.y << 32);
+            cache[i].size = (uint64_t)v.z | ((uint64_t)v.w << 32);
+        }
     if (use_hist)
         for (uint32_t i = tid; i < 2 * n_slots; i += kThreads) hist[i] = 0;
     TmaLane tma;
-    tma.stage = dyn_smem + (size_t)warp * kTmaPiece;
-    tma.bar = &bars[warp];
-    tma.phase = 0;
-    tma.pending = false;
+    tma.stage = dyn_smem + (size_t)warp * kTmaStages * kTmaPiece;
+    tma.bar = &bars[warp * kTmaStages];
+    tma.k = 0;
+    tma.pend_dst = nullptr;
+    tma.pend_len = 0;
+    tma.stores = false;
     if (lane == 0) {
-        mbar_init(tma.bar, 1);
+        for (int s = 0; s < kTmaStages; s++) mbar_init(tma.bar + s, 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     // ================================================================ phase A (a2, a3, a6)
-    for (uint64_t tile = (uint64_t)blockIdx.x * kThreads; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
+    for (uint64_t tile = tile0; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
         const uint64_t i = tile + tid;
-        const bool active = i < a.n;
         uint64_t src = 0, dst = 0, size = 0;
         uint32_t ss = 0, ds = 0;
         bool valid = false;
-        if (active) {
-            const uint4 *p = reinterpret_cast<const uint4 *>(a.descs + i);
-            const uint4 lo = __ldg(p), hi = __ldg(p + 1);
-            ds = lo.x;
-            ss = lo.y;
-            const uint64_t dst_off = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
-            const uint64_t src_off = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
-            size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
-            // destination checked before source; overflow-safe "off + size <= slot size"
-            unsigned bad = 0;
-            SlotRow dr{0, kInvalidSize}, sr{0, kInvalidSize};
-            if (ds < n_slots) dr = a.slots[ds];
-            if (ss < n_slots) sr = a.slots[ss];
-            if (dr.size == kInvalidSize) bad = kBadInvalidSlot;
-            else if (dst_off > dr.size || size > dr.size - dst_off) bad = kBadOutOfBounds;
-            else if (sr.size == kInvalidSize) bad = kBadInvalidSlot;
-            else if (src_off > sr.size || size > sr.size - src_off) bad = kBadOutOfBounds;
+        if (i < a.n) {
+            if (tile != tile0) load_desc_raw(a.descs + i, alo, ahi);
+            const unsigned bad = resolve(alo, ahi, cache, a.slots, n_slots, ds, ss, dst, src, size);
             if (bad) report_bad(ctl, i, bad);
-            else {
-                valid = true;
-                dst = dr.base + dst_off;
-                src = sr.base + src_off;
-            }
+            else valid = true;
         }
 
         // ---- (a6) one message per descriptor: sent on the source slot, recv on the destination
@@ -181,20 +264,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             if (valid && lane == __ffs(md) - 1) atomicAdd(&hist[n_slots + ds], __popc(md));
         }
 
-        // ---- (a3) binning: warp ballot + prefix sums, one atomic per warp per queue
-        const bool is_small = valid && size <= kSmallMax && size > 0;   // zero-size descriptors move nothing
+        // ---- (a3) binning.  Small descriptors (0 < size <= kSmallMax) stay in the table and are
+        // copied from it in place; large ones are expanded into the chunk queue: warp ballot,
+        // warp prefix sum of the chunk counts, one atomic per warp.
         const bool is_large = valid && size > kSmallMax;
-        const unsigned small_mask = __ballot_sync(0xffffffffu, is_small);
-        if (small_mask) {
-            unsigned base = 0;
-            if (lane == 0) base = atomicAdd(&ctl->n_small, __popc(small_mask));
-            base = __shfl_sync(0xffffffffu, base, 0);
-            if (is_small) {
-                const uint64_t pos = base + __popc(small_mask & ((1u << lane) - 1));
-                if (pos < a.small_cap) put_item(a.small_q + pos, src, dst, size);
-                else report_bad(ctl, i, kBadNoCapacity);
-            }
-        }
         const unsigned large_mask = __ballot_sync(0xffffffffu, is_large);
         if (large_mask) {
             const unsigned nch = is_large ? chunk_count(dst, size) : 0u;
@@ -230,16 +303,35 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         }
     }
 
+    // ---- warp tickets of phase B2, set up before the barrier so that their latencies hide
+    // behind it: the first ticket of every warp is static (warp g owns descriptors
+    // [g c0, (g+1) c0)), the second is already an atomic on the shared cursor, which counts
+    // from the end of the static tickets.  Tickets are index ranges only; nothing is copied
+    // before the batch is known to be valid.
+    const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
+    const unsigned gdiv = a.gss * nw, gmax = a.max_group;
+    auto ticket_size = [&](unsigned seen) { return min(max((n - min(seen, n)) / gdiv, 1u), gmax); };
+    const unsigned cnt_static = ticket_size(0), static_end = nw * cnt_static;
+    unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0, cnt1 = 0;
+    if (lane == 0) {
+        cnt1 = ticket_size(static_end);
+        first1 = static_end + atomicAdd(&ctl->next_desc, cnt1);
+    }
+    uint4 flo = make_uint4(0, 0, 0, 0), fhi = flo;
+    const bool fhave = (unsigned)lane < cnt_static && first0 + lane < n;
+    if (fhave) load_desc_raw(a.descs + first0 + lane, flo, fhi);
+
     // ================================================================ grid barrier
+    TRACE(1);
     __syncthreads();
     if (tid == 0) {
-        __threadfence();
-        atomicAdd(&ctl->arrive, 1u);
+        red_release_u32(&ctl->arrive);
         while (ld_acquire_u32(&ctl->arrive) < gridDim.x) {}
     }
     __syncthreads();
     const bool ok = __ldcg(&ctl->bad_inv) == 0;
     if (blockIdx.x == 0 && tid == 0) ctl->t_mid = globaltimer();
+    TRACE(2);
 
     if (ok) {
         // ============================================================ counters (a6)
@@ -266,18 +358,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             }
         }
 
-        // ============================================================ phase B (a4, a5)
-        const unsigned n_chunk = __ldcg(&ctl->n_chunk), n_small = __ldcg(&ctl->n_small);
-        const unsigned n_tickets = n_chunk + (n_small + kWarps - 1) / kWarps;
-        if (tid == 0) sh_ticket[0] = atomicAdd(&ctl->ticket, 1u);
-        __syncthreads();
-        int par = 0;
-        while (true) {
-            const unsigned t = sh_ticket[par];
-            if (t >= n_tickets) break;
-            if (tid == 0) sh_ticket[par ^ 1] = atomicAdd(&ctl->ticket, 1u);   // next round's ticket, a round ahead
-            if (t < n_chunk) {
-                // (a5) the whole CTA copies one chunk
+        // ============================================================ phase B1 (a5): CTA per chunk
+        // dynamic tickets, one atomic per CTA per chunk, fetched one round ahead
+        const unsigned n_chunk = __ldcg(&ctl->n_chunk);
+        if (n_chunk) {
+            if (tid == 0) sh_ticket[0] = atomicAdd(&ctl->ticket, 1u);
+            __syncthreads();
+            int par = 0;
+            while (true) {
+                const unsigned t = sh_ticket[par];
+                if (t >= n_chunk) break;
+                if (tid == 0) sh_ticket[par ^ 1] = atomicAdd(&ctl->ticket, 1u);
                 const WorkItem w = load_item(a.chunk_q + t);
                 unsigned char *d = reinterpret_cast<unsigned char *>(w.dst);
                 const unsigned char *s = reinterpret_cast<const unsigned char *>(w.src);
@@ -287,75 +378,99 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
                 } else {
                     copy_span<kUnroll, kLdDefault, uint32_t, kUnrollShifted>(d, s, (uint32_t)w.size, tid, kThreads);
                 }
-            } else {
-                // (a4) one warp per small descriptor
-                const unsigned i = (t - n_chunk) * kWarps + warp;
-                if (i < n_small) {
-                    const WorkItem w = load_item(a.small_q + i);
-                    unsigned char *d = reinterpret_cast<unsigned char *>(w.dst);
-                    const unsigned char *s = reinterpret_cast<const unsigned char *>(w.src);
-                    if (((w.src | w.dst | w.size) & 15) == 0 && w.size >= a.tma_min) {
-                        if (lane == 0) tma_copy_pieces(tma, d, s, w.size, 0, 1);
-                        __syncwarp();
-                    } else {
-                        copy_span<kUnroll, kLdDefault, uint32_t, kUnrollShifted>(d, s, (uint32_t)w.size, lane, 32);
-                    }
-                }
+                __syncthreads();
+                par ^= 1;
             }
-            __syncthreads();
-            par ^= 1;
         }
+
+        // ============================================================ phase B2 (a4): warp per small descriptor
+        // Small descriptors are read from the table in place.  Each warp takes tickets of
+        // `cnt` consecutive descriptors (one per lane) by guided self-scheduling: a ticket is
+        // 1/(gss x warps) of what is left, at most 32 and at least 1, so the last tickets are
+        // single descriptors and the tail is short.  Three tickets are in flight per warp:
+        // k is being copied, the descriptors of k+1 are being loaded, the atomic of k+2 is
+        // on its way, so neither latency is exposed between two copies.
+        TRACE(3);
+        first1 = __shfl_sync(0xffffffffu, first1, 0);
+        cnt1 = __shfl_sync(0xffffffffu, cnt1, 0);
+        uint64_t src = 0, dst = 0;
+        unsigned sz32 = fhave ? resolve_small(flo, fhi, cache, a.slots, n_slots, dst, src) : 0u;
+        uint4 nlo = make_uint4(0, 0, 0, 0), nhi = nlo;
+        bool nhave = (unsigned)lane < cnt1 && first1 + lane < n;
+        if (nhave) load_desc_raw(a.descs + first1 + lane, nlo, nhi);
+        while (first0 < n) {
+            unsigned first2 = 0, cnt2 = 0;
+            if (lane == 0) {
+                cnt2 = ticket_size(first1 + cnt1);
+                first2 = static_end + atomicAdd(&ctl->next_desc, cnt2);
+            }
+            unsigned m = __ballot_sync(0xffffffffu, sz32 != 0);
+            while (m) {
+                const int l = __ffs(m) - 1;
+                m &= m - 1;
+                const uint64_t s0 = __shfl_sync(0xffffffffu, src, l);
+                const uint64_t d0 = __shfl_sync(0xffffffffu, dst, l);
+                const unsigned z = __shfl_sync(0xffffffffu, sz32, l);
+                unsigned char *d = reinterpret_cast<unsigned char *>(d0);
+                const unsigned char *s = reinterpret_cast<const unsigned char *>(s0);
+                // 16 B vector loads and stores for every alignment; for spans this short the bulk
+                // path measured slower and erratic (one driver lane per warp, S5)
+                copy_span<kUnroll, kLdDefault, uint32_t, kUnrollShifted>(d, s, z, lane, 32);
+            }
+            // rotate: k+1 becomes current (its descriptors have landed), k+2 starts loading
+            sz32 = nhave ? resolve_small(nlo, nhi, cache, a.slots, n_slots, dst, src) : 0u;
+            first0 = first1;
+            first1 = __shfl_sync(0xffffffffu, first2, 0);
+            cnt1 = __shfl_sync(0xffffffffu, cnt2, 0);
+            nhave = (unsigned)lane < cnt1 && first1 + lane < n;
+            if (nhave) load_desc_raw(a.descs + first1 + lane, nlo, nhi);
+        }
+        TRACE(4);
         if (lane == 0) tma_drain(tma);
     }
 
     // ================================================================ finish (feeds a7)
     __syncthreads();
-    if (tid == 0) {
-        __threadfence();
-        sh_flag = atomicAdd(&ctl->done, 1u) == gridDim.x - 1;
-    }
+    TRACE(5);
+    if (tid == 0) sh_flag = atom_inc_acq_rel_u32(&ctl->done) == gridDim.x - 1;
     __syncthreads();
+    TRACE(6);
     if (!sh_flag) return;
-    // last CTA: every CTA's copies and counter updates are complete and visible
-    __threadfence();
+    // last CTA: every CTA's copies and counter updates are complete and visible on the device
+    // (release increments above, acquired by this CTA's thread 0 and handed on by the barrier).
+    // Publish the cumulative counters and the completion record as flagged 8-byte words.
     for (uint32_t s = tid; s < a.n_push; s += kThreads) {
-        a.push[s] = __ldcg(&a.sent[s]);
-        a.push[kPushSlots + s] = __ldcg(&a.recv[s]);
+        const unsigned long long sv = __ldcg(&a.sent[s]), rv = __ldcg(&a.recv[s]);
+        unsigned long long *w = a.push + (size_t)s * kPushWordsPerSlot;
+        put_word(w + 0, (uint32_t)sv, a.flag);
+        put_word(w + 1, (uint32_t)(sv >> 32), a.flag);
+        put_word(w + 2, (uint32_t)rv, a.flag);
+        put_word(w + 3, (uint32_t)(rv >> 32), a.flag);
     }
-    __threadfence_system();
-    __syncthreads();
     if (tid == 0) {
-        HostRecord *r = a.rec;
-        r->bad_inv = __ldcg(&ctl->bad_inv);
-        r->n_small = __ldcg(&ctl->n_small);
-        r->n_chunk = __ldcg(&ctl->n_chunk);
-        r->t_start = __ldcg(&ctl->t_start);
-        r->t_mid = __ldcg(&ctl->t_mid);
-        r->t_end = globaltimer();
+        const unsigned long long bad = __ldcg(&ctl->bad_inv), t0 = __ldcg(&ctl->t_start), t1 = __ldcg(&ctl->t_mid),
+                                 t2 = globaltimer();
+        put_word(a.rec + kRwBadLo, (uint32_t)bad, a.flag);
+        put_word(a.rec + kRwBadHi, (uint32_t)(bad >> 32), a.flag);
+        put_word(a.rec + kRwNChunk, __ldcg(&ctl->n_chunk), a.flag);
+        put_word(a.rec + kRwTStartLo, (uint32_t)t0, a.flag);
+        put_word(a.rec + kRwTStartHi, (uint32_t)(t0 >> 32), a.flag);
+        put_word(a.rec + kRwTMidLo, (uint32_t)t1, a.flag);
+        put_word(a.rec + kRwTMidHi, (uint32_t)(t1 >> 32), a.flag);
+        put_word(a.rec + kRwTEndLo, (uint32_t)t2, a.flag);
+        put_word(a.rec + kRwTEndHi, (uint32_t)(t2 >> 32), a.flag);
         // self-clean: the next batch on the stream finds an all-zero control block
         ctl->bad_inv = 0;
-        ctl->n_small = 0;
         ctl->n_chunk = 0;
         ctl->arrive = 0;
         ctl->ticket = 0;
+        ctl->next_desc = 0;
         ctl->done = 0;
-        __threadfence_system();
-        *reinterpret_cast<volatile unsigned long long *>(&r->seq) = a.seq;
     }
 }
 
 static int ensure_queues(hicr_ctx *ctx, uint64_t n)
 {
-    if (n > ctx->small_cap) {
-        uint64_t cap = std::max<uint64_t>(n, 4096);
-        cap = std::max(cap, ctx->small_cap * 2);
-        HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-        if (ctx->d_small) HICR_CUDA(ctx, cudaFree(ctx->d_small));
-        ctx->d_small = nullptr;
-        ctx->small_cap = 0;
-        HICR_CUDA(ctx, cudaMalloc(&ctx->d_small, cap * sizeof(WorkItem)));
-        ctx->small_cap = cap;
-    }
     // With pairwise-disjoint destinations (the epoch precondition) a batch expands into
     // at most 2 n + registered_bytes / kChunkBytes chunks (a first and a last partial one
     // per descriptor).
@@ -395,20 +510,30 @@ static int get_stage(hicr_ctx *ctx, size_t bytes, StageBlock *out)
 
 size_t engine_smem_bytes(uint32_t n_slots)
 {
-    return (size_t)kWarps * kTmaPiece + (n_slots <= kSmemSlotHist ? 2 * (size_t)n_slots * sizeof(unsigned) : 0);
+    return kSmemStages + kSmemCache + (n_slots <= kSmemSlotHist ? 2 * (size_t)n_slots * sizeof(unsigned) : 0);
 }
 
 // Co-resident CTAs of the engine kernel (what a cooperative launch may use).
 int engine_setup(hicr_ctx *ctx)
 {
     int per_sm = 0;
+    HICR_CUDA(ctx, cudaFuncSetAttribute(engine_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        (int)engine_smem_bytes(kSmemSlotHist)));
     HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, engine_kernel, kThreads,
                                                                  engine_smem_bytes(kSmemSlotHist)));
     if (per_sm < 1) return HICR_ERR_NO_CAPACITY;
-    ctx->engine_grid = ctx->num_sms * std::min(per_sm, kCtasPerSm);
+    per_sm = std::min(per_sm, kCtasPerSm);
+    // tuning overrides (experiments only; the defaults are what is measured and tested)
     const char *e = getenv("HICR_TMA_MIN");
     if (e && *e) ctx->tma_min = (uint32_t)strtoul(e, nullptr, 0);
     if (ctx->tma_min < 16) ctx->tma_min = 16;
+    e = getenv("HICR_CTAS_PER_SM");
+    if (e && *e) per_sm = std::max(1, std::min(per_sm, atoi(e)));
+    e = getenv("HICR_GSS");
+    if (e && *e) ctx->gss = (uint32_t)std::max(1, atoi(e));
+    e = getenv("HICR_MAX_GROUP");
+    if (e && *e) ctx->max_group = (uint32_t)std::max(1, std::min((int)kMaxGroup, atoi(e)));
+    ctx->engine_grid = ctx->num_sms * per_sm;
     return HICR_OK;
 }
 
@@ -421,7 +546,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
 {
     if (!ctx || (!descs && n)) return HICR_ERR_INVALID_ARG;
     if (n == 0) return HICR_OK;
-    if (n >= (1ull << 32)) return HICR_ERR_NO_CAPACITY;
+    if (n >= (1ull << 31)) return HICR_ERR_NO_CAPACITY;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
 
     uint64_t units = ~0ull;   // work tickets of the copy phase, when the host knows them
@@ -471,17 +596,16 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     a.n_slots = (uint32_t)ctx->slots.size();
     a.tma_min = ctx->tma_min;
     a.ctl = ctx->d_ctl;
-    a.small_q = ctx->d_small;
-    a.small_cap = ctx->small_cap;
     a.chunk_q = ctx->d_chunk;
     a.chunk_cap = ctx->chunk_cap;
     a.sent = ctx->d_sent;
     a.recv = ctx->d_recv;
-    a.rec = ctx->d_rec + ctx->batches_in_epoch;
-    a.push = reinterpret_cast<unsigned long long *>(ctx->d_rec + kRecRing);
+    a.rec = ctx->d_rec[ctx->batches_in_epoch].w;
+    a.push = ctx->d_rec[kRecRing].w;
     a.n_push = std::min<uint32_t>(a.n_slots, kPushSlots);
-    a.pad = 0;
-    a.seq = ctx->batch_seq + 1;
+    a.flag = rec_flag(ctx->batch_seq + 1);
+    a.gss = ctx->gss;
+    a.max_group = ctx->max_group;
 
     // grid: every co-resident CTA unless the host knows the batch is smaller than that
     uint64_t want = std::max<uint64_t>((n + kThreads - 1) / kThreads, units == ~0ull ? (uint64_t)ctx->engine_grid : units);

@@ -15,20 +15,24 @@
 namespace hicr {
 
 // ---------------------------------------------------------------- tunables / classes
-// size <= kSmallMax  : warp-per-descriptor queue (a4)
-// size >  kSmallMax  : split at kChunkBytes-aligned destination addresses, CTA-per-chunk queue (a5)
+// 0 < size <= kSmallMax : copied in place from the descriptor table, warp per descriptor (a4)
+// size >  kSmallMax     : split at kChunkBytes-aligned destination addresses, CTA-per-chunk queue (a5)
 constexpr uint64_t kSmallMax = 8192;
 constexpr uint64_t kChunkBytes = 32768;
 constexpr int kThreads = 256;              // 8 warps per CTA of the engine kernel
 constexpr int kWarps = kThreads / 32;
-constexpr int kCtasPerSm = 4;              // persistent grid = SMs x kCtasPerSm (<= 64 registers per thread)
-constexpr int kUnroll = 8;                 // 16-byte vectors in flight per lane (aligned source)
-constexpr int kUnrollShifted = 4;          // the same for byte-shifted sources (keeps the kernel at 64 registers)
+constexpr int kCtasPerSm = 2;              // persistent grid = SMs x kCtasPerSm; 16 warps x 4 x 16 B x 32 lanes = 32 KiB of
+                                           // loads in flight per SM is where a 4 KiB page copy peaks on B200 (S5)
+constexpr int kUnroll = 4;                 // 16-byte vectors in flight per lane (aligned source)
+constexpr int kUnrollShifted = 4;          // the same for byte-shifted sources
 constexpr uint32_t kSmemSlotHist = 1024;   // per-CTA shared-memory counter histogram up to this many slots
-constexpr uint32_t kTmaPiece = 4096;       // bytes per bulk copy; one shared-memory stage per warp
+constexpr uint32_t kSlotCache = 256;       // slot-table rows cached in shared memory (larger tables are read from L2)
+constexpr uint32_t kTmaPiece = 4096;       // bytes per bulk copy
+constexpr int kTmaStages = 2;              // shared-memory stages per warp: load of piece k overlaps the store of piece k-1
 constexpr uint32_t kTmaMinDefault = 1024;  // aligned spans of at least this many bytes take the TMA bulk path
 constexpr int kRecRing = 64;               // host completion records (= batches per epoch before an internal drain)
 constexpr uint32_t kPushSlots = 256;       // counters of the first kPushSlots slots are pushed into the record area
+constexpr unsigned kMaxGroup = 32;         // descriptors per warp ticket, at most (one per lane)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
 constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3;
@@ -41,7 +45,7 @@ struct SlotRow {
 };
 constexpr uint64_t kInvalidSize = ~0ull;
 
-// Work item of both copy queues (32 B so that one lane fetches it with two 16 B loads).
+// Item of the chunk queue (32 B so that one lane fetches it with two 16 B loads).
 struct __align__(16) WorkItem {
     uint64_t src;
     uint64_t dst;
@@ -51,30 +55,42 @@ struct __align__(16) WorkItem {
 
 // Device control block of the engine kernel.  All-zero between batches: the last CTA of
 // a batch publishes the host record and then clears it, so consecutive batches on the
-// stream reuse it without any memset.
+// stream reuse it without any memset.  Every word that many CTAs hammer with atomics sits
+// on its own 128-byte line: 2368 warps taking tickets must not delay the grid barrier or
+// the reads that follow it (they did, by up to 3 us, when all of this shared one line).
 struct __align__(128) Ctl {
+    // line 0: written rarely, read by every CTA after the barrier
     unsigned long long bad_inv;   // atomicMax of ~((index << 4) | error id); 0 = no error
     unsigned long long t_start;   // %globaltimer at kernel start (CTA 0)
     unsigned long long t_mid;     // %globaltimer after the grid barrier (CTA 0)
-    unsigned int n_small;         // items in the warp queue
     unsigned int n_chunk;         // items in the CTA queue
-    unsigned int arrive;          // grid barrier between validation/binning and the copies
-    unsigned int ticket;          // dynamic work tickets of the copy phase
-    unsigned int done;            // CTAs that finished the copy phase
-    unsigned int pad[21];
+    unsigned int pad0[25];
+    unsigned int arrive;          // line 1: grid barrier between validation/binning and the copies
+    unsigned int pad1[31];
+    unsigned int ticket;          // line 2: CTA tickets of the chunk queue
+    unsigned int pad2[31];
+    unsigned int next_desc;       // line 3: warp tickets, first descriptor not yet handed out
+    unsigned int pad3[31];
+    unsigned int done;            // line 4: CTAs that finished the copy phase
+    unsigned int pad4[31];
 };
-static_assert(sizeof(Ctl) == 128, "Ctl is one 128-byte line");
+static_assert(sizeof(Ctl) == 640, "Ctl is five 128-byte lines");
 
-// Completion record of one batch, written by the last CTA into mapped pinned host memory;
-// `seq` is written last (after a system-scope fence) and is what hicr_fence polls.
-struct __align__(64) HostRecord {
-    unsigned long long seq;
-    unsigned long long bad_inv;
-    unsigned long long t_start, t_mid, t_end;
-    unsigned int n_small, n_chunk;
-    unsigned long long pad[2];
+// Completion record of one batch in mapped pinned host memory, written by the last CTA
+// and polled by hicr_fence.  Every 8-byte word is {low: 32 bits of payload, high: flag},
+// flag = rec_flag(batch sequence number) != 0.  A naturally aligned 8-byte store is
+// single-copy atomic, so a word whose flag matches carries its payload: no system-scope
+// fence orders the words (each one costs about 1.6 us on the way out, _work/rtbench).
+constexpr int kRecWords = 16;
+enum RecWord { kRwBadLo = 0, kRwBadHi, kRwNChunk, kRwTStartLo, kRwTStartHi, kRwTMidLo, kRwTMidHi, kRwTEndLo, kRwTEndHi,
+               kRwUsed };
+struct __align__(128) HostRecord {
+    unsigned long long w[kRecWords];
 };
-static_assert(sizeof(HostRecord) == 64, "HostRecord is 64 bytes");
+static_assert(sizeof(HostRecord) == 128, "HostRecord is 128 bytes");
+// pushed counters follow the kRecRing records: 4 words per slot (sent lo, sent hi, recv lo, recv hi)
+constexpr int kPushWordsPerSlot = 4;
+__host__ __device__ inline uint32_t rec_flag(uint64_t seq) { return (uint32_t)(seq % 0xffffffffull) + 1u; }
 
 // Channel state in device memory; head and tail on separate 128 B lines so the
 // producer's and the consumer's polls do not share a line.
@@ -253,6 +269,19 @@ __device__ __forceinline__ unsigned long long ld_acquire(const unsigned long lon
     asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
     return v;
 }
+// Release-increment by one thread after a __syncthreads(): the CTA's earlier writes are
+// ordered before it (bar.sync + release cumulativity) without the L1 invalidation that
+// __threadfence() adds.
+__device__ __forceinline__ void red_release_u32(unsigned *p)
+{
+    asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(p) : "memory");
+}
+__device__ __forceinline__ unsigned atom_inc_acq_rel_u32(unsigned *p)
+{
+    unsigned v;
+    asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(v) : "l"(p) : "memory");
+    return v;
+}
 __device__ __forceinline__ void st_release(unsigned long long *p, unsigned long long v)
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -298,39 +327,69 @@ __device__ __forceinline__ void bulk_wait_read_all() { asm volatile("cp.async.bu
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async;" ::: "memory"); }
 
-// State of one warp's bulk-copy driver (lane 0): one kTmaPiece stage and its mbarrier.
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory"); }
+
+// State of one warp's bulk-copy driver (lane 0): a ring of kTmaStages stages of kTmaPiece
+// bytes, one mbarrier each.  Piece k is loaded into stage k % kTmaStages while the store
+// of piece k-1 is still reading its own stage, so a warp keeps one load and one store in
+// flight (measured best at 2 stages x 16 warps per SM for 4 KiB pages, S5).
 struct TmaLane {
-    unsigned char *stage;
-    uint64_t *bar;
-    unsigned phase;     // parity of the next mbarrier completion
-    bool pending;       // a bulk store may still be reading the stage
+    unsigned char *stage;   // kTmaStages x kTmaPiece bytes
+    uint64_t *bar;          // kTmaStages mbarriers
+    unsigned k;             // pieces issued so far
+    unsigned char *pend_dst;   // destination of piece k-1, whose store has not been issued yet
+    unsigned pend_len;         // 0 = nothing pending
+    bool stores;               // any bulk store issued and not yet drained
 };
 
+// Driver lane only.  Issue the store of the pending piece (after its load has landed).
+__device__ __forceinline__ void tma_store_pending(TmaLane &t)
+{
+    if (t.pend_len) {
+        const unsigned kp = t.k - 1, sp = kp % kTmaStages;
+        mbar_wait(t.bar + sp, (kp / kTmaStages) & 1);
+        bulk_s2g(t.pend_dst, t.stage + sp * kTmaPiece, t.pend_len);
+        bulk_commit();
+        t.pend_len = 0;
+        t.stores = true;
+    }
+}
+
+// Driver lane only: one piece of len <= kTmaPiece bytes; dst, src and len multiples of 16.
+// Order per piece (the one that measured best, S5): wait for the load of piece
+// k-1 and issue its store; wait until at most that one store is still reading shared
+// memory (so the stage of piece k-2 is free); issue the load of piece k into it.
+__device__ __forceinline__ void tma_piece(TmaLane &t, unsigned char *dst, const unsigned char *src, unsigned len)
+{
+    const unsigned st = t.k % kTmaStages;
+    tma_store_pending(t);
+    if (t.stores) bulk_wait_read<kTmaStages - 1>();
+    mbar_expect_tx(t.bar + st, len);
+    bulk_g2s(t.stage + st * kTmaPiece, src, len, t.bar + st);
+    t.pend_dst = dst;
+    t.pend_len = len;
+    t.k++;
+}
+
 // Driver lane only: dst[0, n) = src[0, n) for piece indices first, first + stride, ... of
-// kTmaPiece bytes each; dst, src and n are multiples of 16.  Global -> shared (mbarrier
-// complete_tx), then shared -> global (bulk group); the stage is reused once the store has
-// finished READING it, the writes are completed by tma_drain() before the CTA signals done.
+// kTmaPiece bytes each; dst, src and n are multiples of 16.
 __device__ __forceinline__ void tma_copy_pieces(TmaLane &t, unsigned char *dst, const unsigned char *src, uint64_t n,
                                                 unsigned first, unsigned stride)
 {
-    for (uint64_t off = (uint64_t)first * kTmaPiece; off < n; off += (uint64_t)stride * kTmaPiece) {
-        const unsigned len = (unsigned)min((uint64_t)kTmaPiece, n - off);
-        if (t.pending) bulk_wait_read_all();
-        mbar_expect_tx(t.bar, len);
-        bulk_g2s(t.stage, src + off, len, t.bar);
-        mbar_wait(t.bar, t.phase);
-        t.phase ^= 1;
-        bulk_s2g(dst + off, t.stage, len);
-        bulk_commit();
-        t.pending = true;
-    }
+    for (uint64_t off = (uint64_t)first * kTmaPiece; off < n; off += (uint64_t)stride * kTmaPiece)
+        tma_piece(t, dst + off, src + off, (unsigned)min((uint64_t)kTmaPiece, n - off));
 }
+
+// Driver lane only: everything issued so far is written (complete, not only done reading
+// shared memory) and ordered before the generic-proxy release that follows.
 __device__ __forceinline__ void tma_drain(TmaLane &t)
 {
-    if (t.pending) {
-        bulk_wait_all();       // the bulk stores are complete, not only done reading shared memory
-        fence_proxy_async();   // order the async-proxy writes before the generic-proxy release below
-        t.pending = false;
+    tma_store_pending(t);
+    if (t.stores) {
+        bulk_wait_all();
+        fence_proxy_async();
+        t.stores = false;
     }
 }
 
@@ -374,9 +433,7 @@ struct hicr_ctx {
     int last_error = HICR_OK;                // of the last fence, for hicr_fence_error
     uint64_t last_error_batch = 0, last_error_index = 0;
 
-    // work queues
-    hicr::WorkItem *d_small = nullptr;
-    uint64_t small_cap = 0;
+    // chunk queue (large descriptors expanded by the binning phase)
     hicr::WorkItem *d_chunk = nullptr;
     uint64_t chunk_cap = 0;
 
@@ -394,11 +451,15 @@ struct hicr_ctx {
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
     uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
+    uint32_t gss = 3;                        // HICR_GSS: guided self-scheduling divisor of the warp tickets
+    uint32_t max_group = hicr::kMaxGroup;    // HICR_MAX_GROUP: descriptors per warp ticket, at most
 
     bool profiling = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
     bool ev_valid = false;
-    hicr::HostRecord last_rec = {};          // record of the last completed batch (profile_read)
+    uint64_t last_t[3] = {0, 0, 0};          // %globaltimer stamps of the last completed batch (profile_read)
+    uint64_t rec_bad[hicr::kRecRing] = {};   // bad_inv words of the epoch's records, as read at the drain
+    std::vector<uint32_t> push_words = std::vector<uint32_t>(hicr::kPushWordsPerSlot * hicr::kPushSlots);
 };
 
 namespace hicr {
@@ -406,6 +467,9 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what);
 int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
 int engine_setup(hicr_ctx *ctx);
+#ifdef HICR_TRACE
+void trace_dump(const char *path);
+#endif
 }  // namespace hicr
 
 #define HICR_CUDA(ctx, call)                                                   \
