@@ -343,10 +343,15 @@ def run_cuda(args):
         dom = "engine_kernel"          # the one kernel of a step; duration from CUDA events around its launch
         achieved = bps / (kernel_ms[dom] * 1e-3) / 1e9 if kernel_ms[dom] > 0 else 0.0
         traffic = None
-        tp = os.path.join(ROOT, "profiles", "traffic.json")
+        # dram__bytes_read.sum + dram__bytes_write.sum of that kernel per launch, from the
+        # committed `ncu --set full` summary (profiles/traffic.csv), never measured here
+        tp = os.path.join(ROOT, "profiles", "traffic.csv")
         if os.path.exists(tp):
             try:
-                traffic = json.load(open(tp)).get(args.config, {}).get("dram_bytes_per_launch")
+                import csv
+                for row in csv.DictReader(open(tp)):
+                    if row["config"] == args.config and row["kernel"] == dom:
+                        traffic = float(row["dram_bytes_read_per_launch"]) + float(row["dram_bytes_write_per_launch"])
             except Exception:
                 traffic = None
         # CPU oracle beside it, same workload, bounded to about 10 s of CPU work
