@@ -32,7 +32,7 @@ constexpr int kTmaStages = 2;              // shared-memory stages per warp: loa
 constexpr uint32_t kTmaMinDefault = 1024;  // aligned spans of at least this many bytes take the TMA bulk path
 constexpr int kRecRing = 64;               // host completion records (= batches per epoch before an internal drain)
 constexpr uint32_t kPushSlots = 256;       // counters of the first kPushSlots slots are pushed into the record area
-constexpr unsigned kMaxGroup = 32;         // descriptors per warp ticket, at most (one per lane)
+constexpr unsigned kMaxGroup = 32;         // units per warp ticket, at most (one per lane)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
 constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3;
@@ -59,21 +59,29 @@ struct __align__(16) WorkItem {
 // on its own 128-byte line: 2368 warps taking tickets must not delay the grid barrier or
 // the reads that follow it (they did, by up to 3 us, when all of this shared one line).
 struct __align__(128) Ctl {
-    // line 0: written rarely, read by every CTA after the barrier
+    // line 0: written rarely
     unsigned long long bad_inv;   // atomicMax of ~((index << 4) | error id); 0 = no error
     unsigned long long t_start;   // %globaltimer at kernel start (CTA 0)
     unsigned long long t_mid;     // %globaltimer after the grid barrier (CTA 0)
-    unsigned int n_chunk;         // items in the CTA queue
-    unsigned int pad0[25];
-    unsigned int arrive;          // line 1: grid barrier between validation/binning and the copies
-    unsigned int pad1[31];
+    unsigned int pad0[26];
+    // line 1: the grid barrier between validation/binning and the copies, and everything a
+    // CTA must know when it leaves it, in ONE word, so that the poll that sees the last
+    // arrival also delivers the verdict (no second L2 round trip after the barrier):
+    //   bits  0..11  CTAs arrived              bits 12..23  CTAs that saw an invalid descriptor
+    //   bits 24..35  spare                     bits 36..63  items in the chunk queue
+    unsigned long long sync;
+    unsigned int pad1[30];
     unsigned int ticket;          // line 2: CTA tickets of the chunk queue
     unsigned int pad2[31];
-    unsigned int next_desc;       // line 3: warp tickets, first descriptor not yet handed out
+    unsigned int next_desc;       // line 3: warp tickets, first unit not yet handed out
     unsigned int pad3[31];
     unsigned int done;            // line 4: CTAs that finished the copy phase
     unsigned int pad4[31];
 };
+constexpr int kSyncBadShift = 12, kSyncChunkShift = 36;
+constexpr unsigned long long kSyncFieldMask = 0xfffull;
+constexpr unsigned kMaxGrid = 4095;          // engine grid limit imposed by the 12-bit fields
+constexpr uint64_t kMaxChunks = (1ull << 28) - 1;
 static_assert(sizeof(Ctl) == 640, "Ctl is five 128-byte lines");
 
 // Completion record of one batch in mapped pinned host memory, written by the last CTA
@@ -282,6 +290,10 @@ __device__ __forceinline__ unsigned atom_inc_acq_rel_u32(unsigned *p)
     asm volatile("atom.acq_rel.gpu.global.add.u32 %0, [%1], 1;" : "=r"(v) : "l"(p) : "memory");
     return v;
 }
+__device__ __forceinline__ void atom_add_release_u64(unsigned long long *p, unsigned long long v)
+{
+    asm volatile("red.release.gpu.global.add.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
 __device__ __forceinline__ void st_release(unsigned long long *p, unsigned long long v)
 {
     asm volatile("st.release.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
@@ -452,7 +464,8 @@ struct hicr_ctx {
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
     uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
     uint32_t gss = 3;                        // HICR_GSS: guided self-scheduling divisor of the warp tickets
-    uint32_t max_group = hicr::kMaxGroup;    // HICR_MAX_GROUP: descriptors per warp ticket, at most
+    uint32_t max_group = hicr::kMaxGroup;    // HICR_MAX_GROUP: units per warp ticket, at most
+    uint32_t prefetch = 2;                   // HICR_PREFETCH: descriptors per warp whose source goes to L2 before the barrier
 
     bool profiling = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
