@@ -32,6 +32,9 @@ constexpr int kTmaStages = 2;              // shared-memory stages per warp: loa
 constexpr uint32_t kTmaMinDefault = 1024;  // aligned spans of at least this many bytes take the TMA bulk path
 constexpr int kRecRing = 64;               // host completion records (= batches per epoch before an internal drain)
 constexpr uint32_t kPushSlots = 256;       // counters of the first kPushSlots slots are pushed into the record area
+constexpr int kTeam = 4;                   // lanes per team
+constexpr int kTeamVecs = 4;               // 16 B vectors per lane of a team
+constexpr unsigned kTeamMax = 16 * kTeam * kTeamVecs;   // descriptors up to this size (256 B) are copied by teams, 32 / kTeam at a time
 constexpr unsigned kMaxGroup = 32;         // units per warp ticket, at most (one per lane)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
@@ -269,6 +272,54 @@ __device__ __forceinline__ void copy_span(unsigned char *__restrict__ dst, const
     }
     const uint4 *sA = reinterpret_cast<const uint4 *>(src - s);
     copy_body_shifted<US, POL, IDX>(d4, sA, nvec, s >> 2, (s & 3) * 8, lane, warp, nwarps);
+}
+
+// dst[i] = src[i], i < n <= 16 * G * V, by a TEAM of G consecutive lanes, tl = lane within the
+// team.  The teams of a warp run this together, each on its own short span (n may differ per
+// team, 0 included).  Same decomposition as copy_span -- byte head up to the first 16 B
+// boundary of dst, aligned 16 B stores with aligned or byte-shifted loads, byte tail -- but
+// fully predicated and with EVERY load issued before the first store, so a span costs one
+// memory round trip, not one per part.  A shifted destination vector reads the two aligned
+// source vectors that hold its bytes (the second is the neighbour lane's first: an L1 hit);
+// both contain bytes of the span, so nothing outside the source range's 16 B granules is
+// touched.
+template <int G, int V>
+__device__ __forceinline__ void copy_team(unsigned char *__restrict__ dst, const unsigned char *__restrict__ src,
+                                          unsigned n, int tl)
+{
+    constexpr int HB = (15 + G - 1) / G;   // head / tail bytes per lane, at most
+    unsigned head = (16u - (unsigned)(reinterpret_cast<uintptr_t>(dst) & 15)) & 15u;
+    if (head > n) head = n;
+    const unsigned char *s1 = src + head;
+    unsigned char *d1 = dst + head;
+    const unsigned n1 = n - head, nvec = n1 >> 4, tail = n1 & 15u;
+    const unsigned s = (unsigned)(reinterpret_cast<uintptr_t>(s1) & 15);
+    const uint4 *sA = reinterpret_cast<const uint4 *>(s1 - s);
+    uint4 *d4 = reinterpret_cast<uint4 *>(d1);
+    unsigned char hb[HB], tb[HB];
+    uint4 a[V], b[V];
+#pragma unroll
+    for (int k = 0; k < HB; k++) {
+        hb[k] = tb[k] = 0;
+        if (tl + G * k < head) hb[k] = src[tl + G * k];
+        if (tl + G * k < tail) tb[k] = s1[nvec * 16 + tl + G * k];
+    }
+#pragma unroll
+    for (int k = 0; k < V; k++) {
+        a[k] = b[k] = make_uint4(0, 0, 0, 0);
+        if (tl + G * k < nvec) {
+            a[k] = sA[tl + G * k];
+            if (s) b[k] = sA[tl + G * k + 1];
+        }
+    }
+#pragma unroll
+    for (int k = 0; k < HB; k++) {
+        if (tl + G * k < head) dst[tl + G * k] = hb[k];
+        if (tl + G * k < tail) d1[nvec * 16 + tl + G * k] = tb[k];
+    }
+#pragma unroll
+    for (int k = 0; k < V; k++)
+        if (tl + G * k < nvec) d4[tl + G * k] = shift_combine(a[k], b[k], s >> 2, (s & 3) * 8);   // s = 0: a[k] itself
 }
 
 __device__ __forceinline__ unsigned long long ld_acquire(const unsigned long long *p)
