@@ -137,7 +137,9 @@ struct EngineArgs {
     uint32_t max_group;              // units per warp ticket, at most (<= kMaxGroup)
     uint32_t prefetch;               // descriptors per warp whose source is prefetched into L2 before the barrier
     uint32_t skip_barrier;           // the host validated the table and it holds no large descriptor
+    uint32_t hand_out;               // kHandOutVote (device tables), or what the host's own count says
 };
+constexpr uint32_t kHandOutVote = 0, kHandOutDynamic = 1, kHandOutStatic = 2;
 
 // One 8-byte word of the completion record: payload in the low half, flag in the high half.
 __device__ __forceinline__ void put_word(unsigned long long *w, uint32_t payload, uint32_t flag)
@@ -220,6 +222,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     __shared__ unsigned sh_ticket[2];
     __shared__ unsigned sh_flag;
     __shared__ unsigned long long sh_sync;       // the barrier word as the last poll saw it
+    __shared__ unsigned sh_small[2];             // bytes and count of the small descriptors this CTA validated
     __shared__ unsigned char sh_rank[kWarps][32];   // per warp: lane of the r-th team-sized descriptor of the ticket
     SlotRow *cache = reinterpret_cast<SlotRow *>(dyn_smem + kSmemStages);
     unsigned int *hist = reinterpret_cast<unsigned int *>(dyn_smem + kSmemStages + kSmemCache);
@@ -243,6 +246,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         }
     if (use_hist)
         for (uint32_t i = tid; i < 2 * n_slots; i += kThreads) hist[i] = 0;
+    if (tid < 2) sh_small[tid] = 0;
     TmaLane tma;
     tma.stage = dyn_smem + (size_t)warp * kTmaStages * kTmaPiece;
     tma.bar = &bars[warp * kTmaStages];
@@ -266,6 +270,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
 
     // ================================================================ phase A (a2, a3, a6)
     bool bad_seen = false;
+    unsigned small_bytes = 0, small_cnt = 0;
     for (uint64_t tile = tile0; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
         const uint64_t i = tile + tid;
         uint64_t src = 0, dst = 0, size = 0;
@@ -279,6 +284,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
                 bad_seen = true;
             } else valid = true;
         }
+        if (valid && size != 0 && size <= kSmallMax) {
+            small_bytes += ((unsigned)size + 15u) >> 4;   // in 16 B units: a CTA's sum stays below 2^32
+            small_cnt++;
+        }
+
         // ---- (a6) one message per descriptor: sent on the source slot, recv on the destination
         // (lanes with the same slot elect one leader; invalid lanes carry a key no slot has)
         if (use_hist) {
@@ -329,11 +339,22 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             }
         }
     }
+    // this CTA's vote on how phase B2 hands out work: are its small descriptors team-sized on average?
+#pragma unroll
+    for (int d = 16; d; d >>= 1) {
+        small_bytes += __shfl_xor_sync(0xffffffffu, small_bytes, d);
+        small_cnt += __shfl_xor_sync(0xffffffffu, small_cnt, d);
+    }
+    if (lane == 0 && small_cnt) {
+        atomicAdd(&sh_small[0], small_bytes);
+        atomicAdd(&sh_small[1], small_cnt);
+    }
+
     // the second ticket of every warp and the descriptors of the first are requested before
     // the barrier so that their latencies hide behind it.  Tickets are index ranges only;
     // nothing is written before the batch is known to be valid.
     unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0, cnt1 = 0;
-    if (lane == 0) {
+    if (lane == 0 && a.hand_out != kHandOutStatic) {
         cnt1 = ticket_size(n, static_end);
         first1 = static_end + atomicAdd(&ctl->next_desc, cnt1);
     }
@@ -356,7 +377,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         __syncthreads();
     } else {
         const int cta_bad = __syncthreads_or(bad_seen);
-        if (tid == 0) atom_add_release_u64(&ctl->sync, 1ull | ((unsigned long long)(cta_bad != 0) << kSyncBadShift));
+        if (tid == 0) {
+            const unsigned long long vote = sh_small[1] != 0 && sh_small[0] <= (unsigned long long)(kTeamMax / 16) * sh_small[1];
+            atom_add_release_u64(&ctl->sync, 1ull | ((unsigned long long)(cta_bad != 0) << kSyncBadShift) |
+                                                 (vote << kSyncVoteShift));
+        }
         // While the barrier fills, the sources of the first descriptors this warp will copy start
         // moving into L2, one 128-byte line per lane: the DRAM would otherwise idle until the
         // barrier is through, and reading a source range that passed its own checks has no
@@ -444,12 +469,32 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         TRACE(3);
         first1 = __shfl_sync(0xffffffffu, first1, 0);
         cnt1 = __shfl_sync(0xffffffffu, cnt1, 0);
+        // Team-sized descriptors (the CTAs' votes, or the host's own count) are latency-bound, not
+        // bandwidth-bound: equal counts are balanced enough, and 2368 warps drawing tickets from
+        // one cursor would serialise on it (measured: 5-10 us per batch of 65,536).  They are
+        // handed out statically: after its first ticket warp g owns the g-th share of the rest.
+        const unsigned voters = min((unsigned)gridDim.x, (n + kThreads - 1) / kThreads);
+        const bool static_mode = a.hand_out == kHandOutVote ? 2 * (unsigned)((sync >> kSyncVoteShift) & kSyncFieldMask) >= voters
+                                                            : a.hand_out == kHandOutStatic;
+        unsigned cur = 0, my_hi = 0;
+        if (static_mode) {
+            const unsigned rest = n - min(n, static_end), share = (rest + nw - 1) / nw;
+            cur = min(n, static_end + (blockIdx.x * kWarps + warp) * share);
+            my_hi = min(n, cur + share);
+            cnt1 = min(32u, my_hi - cur);
+            first1 = cnt1 ? cur : n;
+            cur += cnt1;
+        }
         uint4 nlo = make_uint4(0, 0, 0, 0), nhi = nlo;
         bool nhave = (unsigned)lane < cnt1 && first1 + lane < n;
         if (nhave) load_desc_raw(a.descs + first1 + lane, nlo, nhi);
         while (first0 < n) {
             unsigned first2 = 0, cnt2 = 0;
-            if (lane == 0) {
+            if (static_mode) {
+                cnt2 = min(32u, my_hi - cur);
+                first2 = cnt2 ? cur : n;
+                cur += cnt2;
+            } else if (lane == 0) {
                 cnt2 = ticket_size(n, first1 + cnt1);
                 first2 = static_end + atomicAdd(&ctl->next_desc, cnt2);
             }
@@ -634,6 +679,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     uint64_t units = ~0ull;   // work tickets of the copy phase, when the host knows them
     const hicr_desc_t *d_descs = descs;
     bool skip_barrier = false;
+    uint32_t hand_out = kHandOutVote;
     if (!descs_on_device) {
         // (a2) host-resident table: validated here, all-or-nothing, lowest bad index.  One pass
         // checks a descriptor and copies it into pinned staging; the table travels in pieces of
@@ -645,7 +691,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         int rc = get_stage(ctx, n * sizeof(hicr_desc_t), &b);
         if (rc != HICR_OK) return rc;
         hicr_desc_t *stage = static_cast<hicr_desc_t *>(b.host);
-        uint64_t ns = 0, nc = 0;
+        uint64_t ns = 0, nc = 0, small_bytes = 0;
         const size_t nslots = ctx->slots.size();
         const SlotRow *rows = ctx->slots.data();
         for (uint64_t p0 = 0; p0 < n; p0 += kStagePiece) {
@@ -660,7 +706,10 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
                     return rc1;
                 }
                 if (d.size > kSmallMax) nc += d.size / kChunkBytes + 2;
-                else if (d.size) ns++;
+                else if (d.size) {
+                    ns++;
+                    small_bytes += d.size;
+                }
                 stage[i] = d;
             }
             cudaError_t e = cudaMemcpyAsync(static_cast<hicr_desc_t *>(b.dev) + p0, stage + p0, (p1 - p0) * sizeof(hicr_desc_t),
@@ -676,6 +725,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         // checked against the host mirror of the slot table, which the device copy follows in
         // stream order: with no chunk queue to wait for either, the kernel needs no barrier
         skip_barrier = nc == 0;
+        hand_out = ns && small_bytes <= kTeamMax * ns ? kHandOutStatic : kHandOutDynamic;
     }
 
     if (ctx->batches_in_epoch == kRecRing) {
@@ -704,6 +754,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     a.max_group = ctx->max_group;
     a.prefetch = ctx->prefetch;
     a.skip_barrier = skip_barrier ? 1u : 0u;
+    a.hand_out = hand_out;
 
     // grid: every co-resident CTA unless the host knows the batch is smaller than that
     uint64_t want = std::max<uint64_t>((n + kThreads - 1) / kThreads, units == ~0ull ? (uint64_t)ctx->engine_grid : units);

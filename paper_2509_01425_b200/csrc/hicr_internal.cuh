@@ -71,7 +71,8 @@ struct __align__(128) Ctl {
     // CTA must know when it leaves it, in ONE word, so that the poll that sees the last
     // arrival also delivers the verdict (no second L2 round trip after the barrier):
     //   bits  0..11  CTAs arrived              bits 12..23  CTAs that saw an invalid descriptor
-    //   bits 24..35  spare                     bits 36..63  items in the chunk queue
+    //   bits 24..35  CTAs whose small descriptors are team-sized on average (static hand-out)
+    //   bits 36..63  items in the chunk queue
     unsigned long long sync;
     unsigned int pad1[30];
     unsigned int ticket;          // line 2: CTA tickets of the chunk queue
@@ -81,7 +82,7 @@ struct __align__(128) Ctl {
     unsigned int done;            // line 4: CTAs that finished the copy phase
     unsigned int pad4[31];
 };
-constexpr int kSyncBadShift = 12, kSyncChunkShift = 36;
+constexpr int kSyncBadShift = 12, kSyncVoteShift = 24, kSyncChunkShift = 36;
 constexpr unsigned long long kSyncFieldMask = 0xfffull;
 constexpr unsigned kMaxGrid = 4095;          // engine grid limit imposed by the 12-bit fields
 constexpr uint64_t kMaxChunks = (1ull << 28) - 1;
