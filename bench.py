@@ -81,6 +81,16 @@ def shard_report(per_rank_bytes, per_rank_descs, elapsed_ms_max, steps):
     }
 
 
+def rank_max(x: float, dist=None, device="cpu") -> float:
+    """Max over ranks of a per-rank time (the job's time is the slowest rank's)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(x)
+    import torch
+    t = torch.tensor([x], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 # --------------------------------------------------------------------------- clocks
 class ClockSampler:
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
@@ -323,14 +333,7 @@ def run_cuda(args):
         ms_e2e = g0.elapsed_time(g1)
         counters = [ctx.slot_counters(s) for s in ids]
 
-    def allmax(x):
-        if dist is None:
-            return x
-        t = torch.tensor([x], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        return float(t.item())
-
-    ms_max, ms_e2e_max = allmax(ms), allmax(ms_e2e)
+    ms_max, ms_e2e_max = rank_max(ms, dist, "cuda"), rank_max(ms_e2e, dist, "cuda")
     bps, dps = bytes_per_step(w), descs_per_step(w)
     agg = shard_report([bps * K] * world, [dps * K] * world, ms_max, K)
     agg_e2e = shard_report([bps * K] * world, [dps * K] * world, ms_e2e_max, K)
