@@ -393,18 +393,125 @@ def run_cuda(args):
     return 0
 
 
+# --------------------------------------------------------------------------- channel configs
+CHANNEL_TEXT = {
+    "spsc_stream": "config 5a SPSC, device-resident run: 256 B tokens, capacity 1024, 2^24 tokens, batches U{1..1024}, "
+                   "producer CTA and consumer CTA in one kernel",
+    "spsc_calls": "config 5a SPSC, host-call path: push(b_i) then pop(max = capacity), one launch per call",
+    "mpsc": "config 5b non-locking MPSC: 148 producers (one CTA per SM), 64 B tokens, 2^20 tokens each, rings of 1024, "
+            "single consumer CTA",
+}
+
+
+def run_channel(args):
+    """Configs 5a / 5b.  A step is the whole push/pop sequence; bytes = 4 x payload (source ->
+    ring -> sink, read + write each hop).  value = device time of the sequence; e2e = the
+    same through the host-call API where there is one (spsc_calls), else the same number
+    with the host wall clock around the blocking call."""
+    import torch
+    import paper_2509_01425_b200 as hicr
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    K, Wm = args.steps, max(1, args.warmup)
+    name = args.config
+    if name == "mpsc":
+        w = W.mpsc() if args.tokens is None else W.mpsc(n_tokens=args.tokens)
+    else:
+        w = W.spsc() if args.tokens is None else W.spsc(n_tokens=args.tokens)
+    T, C, P, N = w.token_bytes, w.capacity, w.producers, w.n_tokens
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream):
+        ctx = hicr.Context(0, stream.cuda_stream)
+        rings = [torch.zeros(T * C, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        srcs = [torch.from_numpy(w.source_image(p)).cuda() for p in range(P)]
+        sinks = [torch.zeros(N * T, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        rid = [ctx.slot_register(t) for t in rings]
+        sid = [ctx.slot_register(t) for t in srcs]
+        kid = [ctx.slot_register(t) for t in sinks]
+        stream.synchronize()
+        if name == "mpsc":
+            m = ctx.mpsc_create(rid, T, C)
+            def step():
+                m.stream(sid, kid, N, 256)
+        else:
+            ch = ctx.channel_create(rid[0], T, C)
+            batches = w.batches[0]
+            if name == "spsc_stream":
+                def step():
+                    ch.stream(sid[0], 0, kid[0], 0, batches)
+            else:
+                def step():
+                    pos = 0
+                    for b in batches:
+                        b = int(b)
+                        k = ch.push(sid[0], pos * T, b)
+                        k2 = ch.pop(kid[0], pos * T, C)
+                        assert k == b == k2
+                        pos += b
+        for _ in range(Wm):
+            step()
+        clocks = ClockSampler(0)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        l0 = ctx.launch_count()
+        clocks.start()
+        t0 = time.perf_counter()
+        e0.record(stream)
+        for _ in range(K):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        t_host = time.perf_counter() - t0
+        clk = clocks.stop()
+        launches = ctx.launch_count() - l0
+        ms = e0.elapsed_time(e1)
+        ok = all(torch.equal(a, b) for a, b in zip(srcs, sinks))
+    tokens = float(P) * N
+    bytes_step = 4.0 * tokens * T
+    peak, peak_src = load_peaks()
+    gbs = bytes_step * K / (ms * 1e-3) / 1e9
+    line = {
+        "metric": METRIC, "value": gbs, "unit": UNIT, "n_gpus": 1, "steps": K, "warmup": Wm, "ms_per_step": ms / K,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": CHANNEL_TEXT[name], "name": name, "tokens": int(tokens), "token_bytes": T,
+                   "l2": "inputs larger than L2: %d MiB of source and sink per step" % (2 * tokens * T / 2 ** 20)},
+        "tokens_per_s": tokens * K / (ms * 1e-3),
+        "e2e": {"value": bytes_step * K / t_host / 1e9, "unit": UNIT,
+                "h2d_bytes_per_step": int(8 * len(w.batches[0])) if name == "spsc_stream" else 0,
+                "d2h_bytes_per_step": 32 * (2 * len(w.batches[0]) if name == "spsc_calls" else 1),
+                "ms_per_step": 1e3 * t_host / K, "what": "host wall clock around the blocking calls"},
+        "gpu_launches": int(launches),
+        "roofline": {"bound": "hbm", "kernel": "spsc_stream_kernel" if name != "mpsc" else "mpsc_stream_kernel",
+                     "achieved": gbs / 2, "peak": peak, "unit": UNIT, "frac": gbs / 2 / peak, "traffic": None,
+                     "peak_source": peak_src,
+                     "note": "DRAM sees source and sink only (the ring lives in L2): algorithmic DRAM bytes = 2 x payload; "
+                             "the bound that binds is one producer CTA and one consumer CTA per ring, not HBM"},
+        "cpu_baseline": None, "clocks": clk, "sink_equals_source": bool(ok),
+    }
+    print(json.dumps(line))
+    ctx.close()
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", default="bulk", choices=sorted(WORKLOAD_TEXT))
+    ap.add_argument("--config", default="bulk", choices=sorted(WORKLOAD_TEXT) + sorted(CHANNEL_TEXT))
+    ap.add_argument("--tokens", type=int, default=None, help="channel configs: tokens per producer (default: full size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU work of the cpu_baseline leg")
     ap.add_argument("--reference-seconds", type=float, default=90.0,
                     help="--impl reference: CPU work of the whole run (each step a bounded sample)")
     args = ap.parse_args(argv)
+    if args.config in CHANNEL_TEXT:
+        if args.impl == "reference":
+            raise SystemExit("--impl reference times the memcpy configs only")
+        args.steps = min(args.steps, 3) if args.steps == 2000 else args.steps
+        return run_channel(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_cuda(args)

@@ -6,6 +6,7 @@
 //                          incoming and outgoing data transfers have been completed"
 #include "hicr_internal.cuh"
 
+#include <algorithm>
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
@@ -212,6 +213,13 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
             return rc;
         }
     }
+    {
+        // host threads for host-resident tables: the caller's plus helpers
+        int threads = 4;
+        const char *e = getenv("HICR_STAGE_THREADS");
+        if (e && *e) threads = std::max(1, std::min(64, atoi(e)));
+        ctx->stage_pool = stage_pool_create(threads - 1);
+    }
     *out = ctx;
     return HICR_OK;
 }
@@ -224,6 +232,8 @@ int hicr_finalize(hicr_ctx_t *ctx)
 #ifdef HICR_TRACE
     if (getenv("HICR_TRACE_FILE")) trace_dump(getenv("HICR_TRACE_FILE"));
 #endif
+    stage_pool_destroy(ctx->stage_pool);
+    stage_done_free(ctx->stage_done);
     cudaFree(ctx->d_slots);
     cudaFree(ctx->d_sent);
     cudaFree(ctx->d_recv);

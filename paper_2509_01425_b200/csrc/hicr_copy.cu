@@ -657,17 +657,6 @@ int engine_setup(hicr_ctx *ctx)
 
 using namespace hicr;
 
-// One descriptor against the host mirror of the slot table: destination before source,
-// overflow-safe "off + size <= slot size" (same order as the device-side resolve()).
-static int check_desc(const hicr_desc_t &d, const SlotRow *rows, size_t nslots)
-{
-    if (d.dst_slot >= nslots || rows[d.dst_slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    if (d.dst_off > rows[d.dst_slot].size || d.size > rows[d.dst_slot].size - d.dst_off) return HICR_ERR_OUT_OF_BOUNDS;
-    if (d.src_slot >= nslots || rows[d.src_slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    if (d.src_off > rows[d.src_slot].size || d.size > rows[d.src_slot].size - d.src_off) return HICR_ERR_OUT_OF_BOUNDS;
-    return HICR_OK;
-}
-
 extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint64_t n, int descs_on_device,
                                  uint64_t *first_bad)
 {
@@ -681,43 +670,19 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     bool skip_barrier = false;
     uint32_t hand_out = kHandOutVote;
     if (!descs_on_device) {
-        // (a2) host-resident table: validated here, all-or-nothing, lowest bad index.  One pass
-        // checks a descriptor and copies it into pinned staging; the table travels in pieces of
-        // kStagePiece descriptors, each sent as soon as it is checked, so the transfer of piece
-        // k overlaps the checks of piece k+1.  A bad descriptor in a later piece leaves earlier
-        // pieces in the staging block, which nothing reads: no kernel is launched.
-        constexpr uint64_t kStagePiece = 16384;
+        // (a2) host-resident table: validated on the host (hicr_stage.cu), all-or-nothing, lowest
+        // bad index.  One pass checks a descriptor and copies it into pinned staging, on a few
+        // host threads; finished prefixes travel to the device while the rest is being checked.
+        // A bad descriptor leaves earlier pieces in the staging block, which nothing reads: no
+        // kernel is launched.
         StageBlock b;
         int rc = get_stage(ctx, n * sizeof(hicr_desc_t), &b);
         if (rc != HICR_OK) return rc;
-        hicr_desc_t *stage = static_cast<hicr_desc_t *>(b.host);
         uint64_t ns = 0, nc = 0, small_bytes = 0;
-        const size_t nslots = ctx->slots.size();
-        const SlotRow *rows = ctx->slots.data();
-        for (uint64_t p0 = 0; p0 < n; p0 += kStagePiece) {
-            const uint64_t p1 = std::min(n, p0 + kStagePiece);
-            // (the loop is bound by host memory bandwidth: a branch-free variant measured slower)
-            for (uint64_t i = p0; i < p1; i++) {
-                const hicr_desc_t d = descs[i];
-                const int rc1 = check_desc(d, rows, nslots);
-                if (rc1 != HICR_OK) {
-                    if (first_bad) *first_bad = i;
-                    ctx->free_stage.push_back(b);
-                    return rc1;
-                }
-                if (d.size > kSmallMax) nc += d.size / kChunkBytes + 2;
-                else if (d.size) {
-                    ns++;
-                    small_bytes += d.size;
-                }
-                stage[i] = d;
-            }
-            cudaError_t e = cudaMemcpyAsync(static_cast<hicr_desc_t *>(b.dev) + p0, stage + p0, (p1 - p0) * sizeof(hicr_desc_t),
-                                            cudaMemcpyHostToDevice, ctx->stream);
-            if (e != cudaSuccess) {
-                ctx->free_stage.push_back(b);
-                return cuda_fail(ctx, e, "cudaMemcpyAsync(descriptor table)");
-            }
+        rc = stage_table(ctx, descs, n, b, first_bad, &nc, &ns, &small_bytes);
+        if (rc != HICR_OK) {
+            ctx->free_stage.push_back(b);
+            return rc;
         }
         units = nc + (ns + kWarps - 1) / kWarps;
         ctx->used_stage.push_back(b);

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <atomic>
 #include <string>
 #include <vector>
 
@@ -468,6 +469,10 @@ struct StageBlock {
 
 }  // namespace hicr
 
+namespace hicr {
+class StagePool;
+}
+
 struct hicr_ctx {
     int device = 0;
     cudaStream_t stream = nullptr;
@@ -504,6 +509,11 @@ struct hicr_ctx {
     // staging of host-resident descriptor tables (returned to `free_stage` at the fence)
     std::vector<hicr::StageBlock> free_stage, used_stage;
 
+    // host threads that check and stage host-resident tables (HICR_STAGE_THREADS, default 4 incl. the caller)
+    hicr::StagePool *stage_pool = nullptr;
+    std::atomic<uint64_t> *stage_done = nullptr;
+    uint64_t stage_done_cap = 0;
+
     // counter read-back for slot tables larger than kPushSlots (pinned)
     unsigned char *h_fence = nullptr;
     size_t h_fence_bytes = 0;
@@ -532,6 +542,12 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what);
 int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
 int engine_setup(hicr_ctx *ctx);
+int check_desc(const hicr_desc_t &d, const SlotRow *rows, size_t nslots);
+int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const StageBlock &b, uint64_t *first_bad,
+                uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
+StagePool *stage_pool_create(int helpers);
+void stage_pool_destroy(StagePool *p);
+void stage_done_free(std::atomic<uint64_t> *p);
 #ifdef HICR_TRACE
 void trace_dump(const char *path);
 #endif
