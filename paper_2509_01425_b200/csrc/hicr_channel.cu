@@ -131,25 +131,25 @@ spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C
     const uint64_t ring_bytes = C * T;
     const int tid = threadIdx.x;
     if (blockIdx.x == 0) {
-        unsigned long long head = st->head;
+        unsigned long long head = st->head, tail_seen = st->tail;   // tail only grows: a stale value is a safe bound
         uint64_t pushed = 0;
         for (uint64_t b = 0; b < n_batches; b++) {
             uint64_t rem = batches[b];
             while (rem) {            // blocking push: wait for room, push what fits
                 if (tid == 0) {
-                    unsigned ns = 20;
-                    unsigned long long room;
-                    while ((room = C - (head - ld_acquire(&st->tail))) == 0) backoff(ns);
+                    unsigned long long room = C - (head - tail_seen);
+                    if (room < rem) {   // look at the consumer's counter only when the known room is short
+                        unsigned ns = 20;
+                        while ((room = C - (head - (tail_seen = ld_acquire(&st->tail)))) == 0) backoff(ns);
+                    }
                     sh_k = min((unsigned long long)rem, room);
                 }
                 __syncthreads();
                 const uint64_t k = sh_k;
                 ring_copy<8, true>(ring, ring_bytes, (head % C) * T, src + pushed * T, k * T, tid, kStreamThreads);
                 __syncthreads();     // every thread's payload stores are issued
-                if (tid == 0) {
-                    __threadfence();
-                    st_release(&st->head, head + k);
-                }
+                // payload before counter: the release covers the CTA's stores ordered before it by the barrier
+                if (tid == 0) st_release(&st->head, head + k);
                 head += k;
                 pushed += k;
                 rem -= k;
@@ -169,10 +169,7 @@ spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C
             const uint64_t k = sh_k;
             ring_copy<8, false>(ring, ring_bytes, (tail % C) * T, dst + popped * T, k * T, tid, kStreamThreads);
             __syncthreads();         // every thread's ring loads have returned (their stores were issued)
-            if (tid == 0) {
-                __threadfence();
-                st_release(&st->tail, tail + k);
-            }
+            if (tid == 0) st_release(&st->tail, tail + k);
             tail += k;
             popped += k;
         }
@@ -219,10 +216,7 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
             const uint64_t k = sh_k;
             ring_copy<2, true>(ring, ring_bytes, (head % C) * T, src + pushed * T, k * T, tid, kMpscThreads);
             __syncthreads();
-            if (tid == 0) {
-                __threadfence();
-                st_release(&s->head, head + k);
-            }
+            if (tid == 0) st_release(&s->head, head + k);
             head += k;
             pushed += k;
         }
@@ -254,7 +248,6 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
             ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
             __syncwarp();
             if (lane == 0) {
-                __threadfence();
                 st_release(&s->tail, tail + k);
                 if (tail + k == tokens) {   // this ring is through: one message per token (reading 15)
                     atomicAdd(&sent[slot_ids[P + p]], (unsigned long long)tokens);

@@ -308,3 +308,48 @@ def test_config3_quarter_size(hicr, variant):
     ref = run_oracle(w)
     got = run_gpu(w, device_tables=True)
     assert_same(w, ref, got)
+
+
+# ------------------------------------------------------------ host tables on several host threads
+def test_large_host_table_parity_and_late_error(hicr):
+    """A host table long enough for the threaded check-and-stage path (hicr_stage.cu: pieces of
+    4096 descriptors claimed by the caller and the helper threads): same image and counters
+    as the oracle; with two bad descriptors in late pieces the LOWEST index is reported,
+    nothing is copied or counted, and the context keeps working."""
+    from oracle import Oracle
+    w = W.bulk_aligned(n_desc=50000, slot_bytes=256 * W.MiB, page=1024, n_sets=1)
+    ref = run_oracle(w)
+    got = run_gpu(w, device_tables=False)
+    assert_same(w, ref, got, "threaded host table")
+
+    bad = w.epochs[0].copy()
+    bad["src_off"][45000] = 2 ** 63                                   # a later piece
+    bad["dst_slot"][30001] = 5                                        # the lowest bad index
+    o = Oracle()
+    for s in range(2):
+        o.slot_register(w.slot_image(s))
+    orc_status, orc_bad = o.memcpy_batch(bad)
+    assert orc_bad == 30001
+    with _ctx(hicr) as ctx:
+        bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(2)]
+        ids = [ctx.slot_register(b) for b in bufs]
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.memcpy_batch(bad)
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT == orc_status
+        assert e.value.first_bad == 30001
+        ctx.fence()
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == w.slot_image(s).tobytes()
+        assert [ctx.slot_counters(s) for s in ids] == [(0, 0), (0, 0)]
+        ctx.memcpy_batch(w.epochs[0])
+        ctx.fence()
+        assert [ctx.slot_counters(s) for s in ids] == [(50000, 0), (0, 50000)]
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == ref[0][s].tobytes()
+
+
+def test_chain_host_tables_static_hand_out(hicr):
+    """Config 4's shape through HOST tables: the host counts the batch as team-sized, so the
+    kernel runs without barrier and with the static hand-out; 6 chained epochs."""
+    w = W.chained_epochs(n_epochs=6, n_desc=20000, slot_bytes=32 * W.MiB)
+    assert_same(w, run_oracle(w), run_gpu(w, device_tables=False), "chain, host tables")
