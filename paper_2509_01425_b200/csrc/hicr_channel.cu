@@ -63,6 +63,61 @@ __device__ __forceinline__ void ring_copy(unsigned char *ring, uint64_t ring_byt
     }
 }
 
+// ---- deep TMA ring of one driver lane: S stages of kTmaPiece bytes, up to S bulk loads in
+// flight ahead of the stores.  The single MPSC consumer has to keep far more bytes in flight
+// than its registers allow: 8 warps x 5 x 2 KiB = 80 KiB here against 16 KiB with 4 vectors
+// per lane.  kl / ks = loads / stores issued so far, ever: stage = k % S, mbarrier parity =
+// (k / S) & 1.
+template <int S, int PIECE>
+struct TmaRing {
+    unsigned char *stage;
+    uint64_t *bar;
+    unsigned kl, ks;
+};
+__device__ __forceinline__ void ring_wait_read(unsigned n)   // at most n of my bulk stores still read shared memory
+{
+    switch (n) {
+    case 0: bulk_wait_read<0>(); break;
+    case 1: bulk_wait_read<1>(); break;
+    case 2: bulk_wait_read<2>(); break;
+    case 3: bulk_wait_read<3>(); break;
+    case 4: bulk_wait_read<4>(); break;
+    default: bulk_wait_read<5>(); break;
+    }
+}
+// Driver lane only: dst[0, n) = src[0, n) in pieces of PIECE bytes; dst, src, n multiples of 16.
+// At most S - 1 loads run ahead of the stores, so the stage a load refills was handed to a
+// store at least one piece ago and the wait for that store's shared-memory read is short.
+// On return every load has landed (the source bytes have been read) and every store has been
+// issued, not necessarily completed.
+template <int S, int PIECE>
+__device__ __forceinline__ void tma_ring_copy(TmaRing<S, PIECE> &r, unsigned char *dst, const unsigned char *src, uint64_t n)
+{
+    static_assert(S >= 2 && S <= 7, "ring_wait_read covers up to 5 stores in flight");
+    const unsigned np = (unsigned)((n + PIECE - 1) / PIECE);
+    unsigned issued = 0, stored = 0;
+    while (stored < np) {
+        while (issued < np && r.kl - r.ks < (unsigned)(S - 1)) {
+            // the stage of load kl was last read by store kl - S; S - 1 - (kl - ks) stores came after it
+            if (r.kl >= (unsigned)S) ring_wait_read(S - 1 - (r.kl - r.ks));
+            const uint64_t off = (uint64_t)issued * PIECE;
+            const unsigned len = (unsigned)min((uint64_t)PIECE, n - off), st = r.kl % S;
+            mbar_expect_tx(r.bar + st, len);
+            bulk_g2s(r.stage + st * PIECE, src + off, len, r.bar + st);
+            r.kl++;
+            issued++;
+        }
+        const uint64_t off = (uint64_t)stored * PIECE;
+        const unsigned len = (unsigned)min((uint64_t)PIECE, n - off), st = r.ks % S;
+        mbar_wait(r.bar + st, (r.ks / S) & 1);
+        bulk_s2g(dst + off, r.stage + st * PIECE, len);
+        bulk_commit();
+        r.ks++;
+        stored++;
+    }
+}
+constexpr int kMpscStages = 3, kMpscPiece = 4096;   // 8 warps x 3 x 4 KiB = 96 KiB: two CTAs per SM stay co-resident
+
 // (a8) push / (a9) pop as one launch.  `lin` = the linear side (source slot for push,
 // destination slot for pop) already offset; lin_room = bytes available there.
 template <bool PUSH>
@@ -192,8 +247,10 @@ spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C
 __global__ void __launch_bounds__(kMpscThreads, 2)
 mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const uint64_t *__restrict__ ptrs,
                    const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch,
-                   unsigned long long *sent, unsigned long long *recv)
+                   unsigned long long *sent, unsigned long long *recv, int use_tma)
 {
+    extern __shared__ __align__(128) unsigned char dyn_smem[];   // consumer, use_tma: [warp][stage][kMpscPiece]
+    __shared__ uint64_t bars[(kMpscThreads / 32) * kMpscStages];
     const uint64_t ring_bytes = C * T;
     const int tid = threadIdx.x;
     if (blockIdx.x < P) {
@@ -224,6 +281,15 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
     }
     // ---- the single consumer: warp w polls and drains rings w, w + nwarps, ...
     const int lane = tid & 31, warp = tid >> 5, nwarps = kMpscThreads / 32;
+    TmaRing<kMpscStages, kMpscPiece> tr;
+    tr.stage = dyn_smem + (size_t)warp * kMpscStages * kMpscPiece;
+    tr.bar = &bars[warp * kMpscStages];
+    tr.kl = tr.ks = 0;
+    if (use_tma && lane == 0) {
+        for (int i = 0; i < kMpscStages; i++) mbar_init(tr.bar + i, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncwarp();
     bool all_done = false;
     unsigned ns = 20;
     while (!all_done) {
@@ -245,7 +311,18 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
             progressed = true;
             unsigned char *ring = reinterpret_cast<unsigned char *>(ptrs[p]);
             unsigned char *dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]);
-            ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
+            if (use_tma) {
+                // bulk copies ring -> shared -> sink, up to kMpscStages loads in flight; when the call
+                // returns the ring bytes have been read, so the tail can move while the stores drain
+                if (lane == 0) {
+                    fence_proxy_async();   // head was acquired in the generic proxy, the copies run in the async one
+                    const uint64_t rb = (tail % C) * T, len = k * T, a = min(len, ring_bytes - rb);
+                    tma_ring_copy<kMpscStages, kMpscPiece>(tr, dst + tail * T, ring + rb, a);
+                    if (len > a) tma_ring_copy<kMpscStages, kMpscPiece>(tr, dst + tail * T + a, ring, len - a);
+                }
+            } else {
+                ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
+            }
             __syncwarp();
             if (lane == 0) {
                 st_release(&s->tail, tail + k);
@@ -259,6 +336,7 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
         }
         if (!progressed && !all_done) backoff(ns); else ns = 20;
     }
+    if (use_tma && lane == 0) bulk_wait_all();   // the sink is complete (and shared memory free) before the CTA exits
 }
 
 // The kernel wrote the result into mapped pinned memory before the stream synchronize returned.
@@ -506,9 +584,24 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_sl
     if (N == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     // co-residency of all P + 1 CTAs is what makes the spin-waits safe
+    // every ring, sink and token size a multiple of 16 bytes: the consumer moves tokens with bulk copies
+    int use_tma = m->T % 16 == 0;
+    for (uint32_t p = 0; p < P && use_tma; p++)
+        use_tma = (ctx->slots[m->rings[p]].base | ctx->slots[dst_slots[p]].base) % 16 == 0;
+    size_t smem = use_tma ? (size_t)(kMpscThreads / 32) * kMpscStages * kMpscPiece : 0;
     int per_sm = 0;
-    HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, 0));
-    if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
+    if (use_tma) {
+        HICR_CUDA(ctx, cudaFuncSetAttribute(mpsc_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, smem));
+        if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) {
+            use_tma = 0;
+            smem = 0;
+        }
+    }
+    if (!use_tma) {
+        HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, 0));
+        if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
+    }
 
     std::vector<uint64_t> ptrs(3 * (size_t)P);
     std::vector<uint32_t> ids(3 * (size_t)P);
@@ -532,9 +625,9 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_sl
     const uint64_t *pp = m->d_ptrs;
     const uint32_t *ip = d_ids;
     unsigned long long *sent = ctx->d_sent, *recv = ctx->d_recv;
-    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &sent, &recv};
+    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &sent, &recv, &use_tma};
     HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_stream_kernel, dim3(P + 1), dim3(kMpscThreads),
-                                               args, 0, ctx->stream));
+                                               args, smem, ctx->stream));
     ctx->launches++;
     HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (uint32_t p = 0; p < P; p++) {
