@@ -117,6 +117,8 @@ class Context:
         self._h = h
         self._keep = {}      # slot id -> object that owns the storage (kept alive)
         self._children = []
+        self._bad = ctypes.c_uint64(0)          # out-argument of hicr_memcpy_batch, reused across calls
+        self._bad_ref = ctypes.byref(self._bad)
 
     # ---- plumbing
     def close(self):
@@ -180,6 +182,11 @@ class Context:
         """hicr_memcpy_batch.  ``descs``: numpy array of DESC_DTYPE (host table), or a
         torch CUDA tensor / int device address of ``n`` 32-byte descriptors (device
         table; must stay alive until the fence)."""
+        if type(descs) is int:                  # device address: the hot path, nothing to marshal
+            rc = lib.hicr_memcpy_batch(self._h, descs, n, 1, self._bad_ref)
+            if rc != HICR_OK:
+                self._fail(rc, "hicr_memcpy_batch", first_bad=self._bad.value)
+            return
         bad = ctypes.c_uint64(0)
         if isinstance(descs, np.ndarray):
             if descs.dtype != DESC_DTYPE or not descs.flags.c_contiguous:
