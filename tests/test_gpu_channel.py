@@ -253,3 +253,56 @@ def test_mpsc_stream(hicr, P, N, T, C, maxb):
     sink = per-producer source, head_p = tail_p = N, independent of the interleaving."""
     w = W.mpsc(producers=P, n_tokens=N, token_bytes=T, capacity=C, max_batch=maxb)
     _mpsc_both(hicr, w, maxb)
+
+
+# ------------------------------------------------------------ full-size configs 5a / 5b
+@pytest.mark.timeout(900)
+def test_config5a_full_size_stream(hicr):
+    """BASELINE.json config 5a at FULL size (2^24 tokens of 256 B, capacity 1024, batches
+    U{1..1024}) through the device-resident run bench.py times; the oracle does the push /
+    pop(max = C) call sequence token by token.  Sink, ring, head/tail and message counters."""
+    w = W.spsc()
+    assert w.n_tokens == 1 << 24 and w.token_bytes == 256 and w.capacity == 1024
+    p = Pair(hicr, w.token_bytes, w.capacity, w.source_image(0), w.n_tokens * w.token_bytes)
+    try:
+        pos = 0
+        for b in w.batches[0]:
+            b = int(b)
+            assert p.o.channel_push(p.och, p.ids[1], pos * p.T, b) == (oracle.OK, b)
+            assert p.o.channel_pop(p.och, p.ids[2], pos * p.T, p.C) == (oracle.OK, b)
+            pos += b
+        assert pos == 1 << 24
+        p.ch.stream(p.ids[1], 0, p.ids[2], 0, w.batches[0])
+        p.check("5a full size")
+        assert p.ch.counters() == (1 << 24, 1 << 24)
+    finally:
+        p.close()
+
+
+@pytest.mark.timeout(900)
+def test_config5b_full_size_properties(hicr):
+    """BASELINE.json config 5b at FULL size (148 producers x 2^20 tokens of 64 B): the result
+    has a plain definition that needs no interleaving -- every sink equals its producer's
+    source (per-producer FIFO), head_p = tail_p = 2^20, one message per token on every
+    slot -- checked on the device for all 9.25 GiB."""
+    w = W.mpsc()
+    T, C, P, N = w.token_bytes, w.capacity, w.producers, w.n_tokens
+    assert (P, N, T) == (148, 1 << 20, 64)
+    with _ctx(hicr) as ctx:
+        rings = [torch.zeros(T * C, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        srcs = [torch.from_numpy(w.source_image(p)).cuda() for p in range(P)]
+        sinks = [torch.zeros(N * T, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        rid = [ctx.slot_register(t) for t in rings]
+        sid = [ctx.slot_register(t) for t in srcs]
+        kid = [ctx.slot_register(t) for t in sinks]
+        m = ctx.mpsc_create(rid, T, C)
+        m.stream(sid, kid, N, 256)
+        torch.cuda.synchronize()
+        for p in range(P):
+            assert m.counters(p) == (N, N)
+            assert torch.equal(sinks[p], srcs[p]), "sink %d" % p
+            # the ring holds the last C tokens, token i at position i mod C (N is a multiple of C)
+            assert torch.equal(rings[p], srcs[p][(N - C) * T:]), "ring %d" % p
+            assert ctx.slot_counters(sid[p]) == (N, 0)
+            assert ctx.slot_counters(rid[p]) == (N, N)
+            assert ctx.slot_counters(kid[p]) == (0, N)

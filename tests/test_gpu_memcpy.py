@@ -353,3 +353,44 @@ def test_chain_host_tables_static_hand_out(hicr):
     kernel runs without barrier and with the static hand-out; 6 chained epochs."""
     w = W.chained_epochs(n_epochs=6, n_desc=20000, slot_bytes=32 * W.MiB)
     assert_same(w, run_oracle(w), run_gpu(w, device_tables=False), "chain, host tables")
+
+
+@pytest.mark.timeout(1800)
+def test_config3a_full_size(hicr):
+    """BASELINE.json config 3 (variant 3a, reading 19) at FULL size -- 64 slots x 256 MiB, 100,000
+    descriptors, one device-resident batch, one fence: the launch configuration bench.py times.
+    The oracle gets the same descriptors one destination slot at a time, against slots trimmed
+    to the zones they touch (the destination slot whole, every slot's 32 MiB source zone), so
+    16 GiB never has to sit in host memory twice; every byte of every slot is compared."""
+    from oracle import Oracle
+    w = W.heavy_tailed("a")
+    d = w.epochs[0]
+    zone = w.meta["src_zone"]
+    n_slots = len(w.slot_sizes)
+    assert int((d["src_off"] + d["size"]).max()) <= zone and int(d["dst_off"].min()) >= zone
+    with _ctx(hicr) as ctx:
+        bufs = []
+        for s in range(n_slots):
+            bufs.append(torch.from_numpy(w.slot_image(s)).cuda())
+        ids = [ctx.slot_register(b) for b in bufs]
+        t = to_device_table(d)
+        ctx.memcpy_batch(t, n=len(d))
+        ctx.fence()
+        got_cnt = [ctx.slot_counters(s) for s in ids]
+        assert ctx.launch_count() == 1
+        sources = [w.slot_image(s)[:zone].copy() for s in range(n_slots)]
+        for s in range(n_slots):
+            sel = d[d["dst_slot"] == s].copy()
+            o = Oracle()
+            img = w.slot_image(s)
+            assert o.slot_register(img) == 0
+            for z in sources:
+                o.slot_register(z)
+            sel["dst_slot"] = 0
+            sel["src_slot"] = sel["src_slot"] + 1
+            assert o.memcpy_batch(np.ascontiguousarray(sel))[0] == 0 and o.fence() == 0
+            assert o.slot_counters(0)[1] == len(sel) == got_cnt[s][1]
+            assert bufs[s].cpu().numpy().tobytes() == img.tobytes(), "slot %d differs from the oracle" % s
+            o.close()
+        sent = np.bincount(d["src_slot"], minlength=n_slots)
+        assert [c[0] for c in got_cnt] == sent.tolist()
