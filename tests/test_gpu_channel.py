@@ -306,3 +306,35 @@ def test_config5b_full_size_properties(hicr):
             assert ctx.slot_counters(sid[p]) == (N, 0)
             assert ctx.slot_counters(rid[p]) == (N, N)
             assert ctx.slot_counters(kid[p]) == (0, N)
+
+
+@pytest.mark.parametrize("s", [1, 7, 4096, (1 << 20) + 3])
+def test_pingpong_capacity_one(hicr, s):
+    """The paper's Test Case 1 shape: two opposing SPSC channels of capacity 1,
+    one message of s bytes bounced A -> B -> A, several rounds; a second push before the pop
+    returns 0 ("may not send any more messages").  Same buffers, rings, head /
+    tail and slot counters as the oracle after every round."""
+    rng = np.random.default_rng(s)
+    imgs = [np.zeros(s, np.uint8), np.zeros(s, np.uint8), rng.integers(0, 256, s, dtype=np.uint8), np.zeros(s, np.uint8)]
+    o = Oracle()
+    oid = [o.slot_register(a) for a in imgs]
+    oab, oba = o.channel_create(oid[0], s, 1)[1], o.channel_create(oid[1], s, 1)[1]
+    with _ctx(hicr) as ctx:
+        g = [torch.from_numpy(a.copy()).cuda() for a in imgs]
+        ids = [ctx.slot_register(t) for t in g]
+        assert ids == oid
+        ab, ba = ctx.channel_create(ids[0], s, 1), ctx.channel_create(ids[1], s, 1)
+        for r in range(3):
+            assert ab.push(ids[2], 0, 1) == 1 == o.channel_push(oab, oid[2], 0, 1)[1]
+            assert ab.push(ids[2], 0, 1) == 0 == o.channel_push(oab, oid[2], 0, 1)[1]      # full
+            assert ab.pop(ids[3], 0, 1) == 1 == o.channel_pop(oab, oid[3], 0, 1)[1]
+            assert ab.pop(ids[3], 0, 1) == 0 == o.channel_pop(oab, oid[3], 0, 1)[1]        # empty
+            assert ba.push(ids[3], 0, 1) == 1 == o.channel_push(oba, oid[3], 0, 1)[1]
+            assert ba.pop(ids[2], 0, 1) == 1 == o.channel_pop(oba, oid[2], 0, 1)[1]
+            assert ab.counters() == o.channel_counters(oab) == (r + 1, r + 1)
+            assert ba.counters() == o.channel_counters(oba) == (r + 1, r + 1)
+        for t, a in zip(g, imgs):
+            assert t.cpu().numpy().tobytes() == a.tobytes()
+        assert imgs[3].tobytes() == imgs[2].tobytes()
+        for i in ids:
+            assert ctx.slot_counters(i) == o.slot_counters(i)
