@@ -54,7 +54,7 @@ def make_workload(name: str, rank: int = 0):
         return W.heavy_tailed("a", seed=seed)
     if name == "heavy_b":
         return W.heavy_tailed("b", seed=seed)
-    if name == "chain":
+    if name in ("chain", "chain_async"):
         return W.chained_epochs(seed=seed)
     raise SystemExit("unknown --config %s" % name)
 
@@ -67,6 +67,8 @@ WORKLOAD_TEXT = {
     "heavy_a": "config 3a heavy-tailed: 64 slots x 256 MiB, 100000 descriptors, power law 1.3 on 16 B..16 MiB",
     "heavy_b": "config 3b heavy-tailed: 64 slots x 256 MiB, log-uniform 16 B..16 MiB until full",
     "chain": "config 4 chained epochs: 1 slot x 256 MiB, 64 epochs x 65536 descriptors of 8..256 B",
+    "chain_async": "config 4 chained epochs with stream-ordered fences (hicr_fence_async) between epochs and ONE blocking "
+                   "fence at the end of the timed region (SURVEY.md S8(f) 3)",
 }
 
 
@@ -269,9 +271,11 @@ def run_cuda(args):
 
         dev_ptrs = [t.data_ptr() for t in dev_tables]
 
+        epoch_fence = ctx.fence_async if args.config == "chain_async" else ctx.fence
+
         def step_device(i):
             ctx.memcpy_batch(dev_ptrs[i % n_sets], n_per[i % n_sets])
-            ctx.fence()
+            epoch_fence()
 
         def step_host(i):
             ctx.memcpy_batch(host_tables[i % n_sets])
@@ -280,6 +284,7 @@ def run_cuda(args):
         # ---- device-resident arm (value): K steps, nothing else on the stream
         for i in range(Wm):
             step_device(i)
+        ctx.fence()
         clocks = ClockSampler(local)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
@@ -289,6 +294,7 @@ def run_cuda(args):
         e0.record(stream)
         for i in range(K):
             step_device(i)
+        ctx.fence()                      # a no-op unless the epochs were closed by stream-ordered fences
         e1.record(stream)
         barrier()
         t_host = time.perf_counter() - t_host0
@@ -302,7 +308,8 @@ def run_cuda(args):
         ctx.profile_enable(True)
         prof = np.zeros(4)
         for i in range(K):
-            step_device(i)
+            ctx.memcpy_batch(dev_ptrs[i % n_sets], n_per[i % n_sets])
+            ctx.fence()
             prof += np.asarray(ctx.profile_read())
         n_prof = K
         ctx.profile_enable(False)

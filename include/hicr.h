@@ -135,6 +135,27 @@ int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint64_t n, int
  * failed one are unaffected. */
 int hicr_fence(hicr_ctx_t *ctx);
 
+/* Stream-ordered fence: closes the epoch WITHOUT blocking the host.  Every
+ * batch enqueued after it is ordered, on the context's stream, after the completion of every
+ * batch enqueued before it, so a later batch may read what an earlier one wrote and the
+ * epoch precondition of hicr_memcpy_batch starts afresh.  Nothing is reported here:
+ * deferred errors, counters and host visibility come with the next blocking hicr_fence /
+ * hicr_fence_expected, whose batch_index then counts batches since the last BLOCKING fence.
+ * (The paper's fence is blocking; this is the asynchronous half of it, for
+ * chains of dependent epochs such as config 4.) */
+int hicr_fence_async(hicr_ctx_t *ctx);
+
+/* Expected-count fence: "suspend execution until the expected number of incoming and outgoing
+ * data transfers have been completed".  Blocks the host until slot `slot` has
+ * cumulatively sent at least `sent` and received at least `recv` messages (counted since
+ * registration, as hicr_slot_counters reports them) AND the transfers counted are complete
+ * and visible.  It does not wait for other outstanding batches and does not close the epoch.
+ * On return hicr_slot_counters of `slot` reports the values seen.  HICR_ERR_INVALID_SLOT on an
+ * unknown slot; HICR_ERR_INVALID_ARG if everything enqueued has completed and the counts are
+ * still short (it would block forever); a deferred error of a completed batch is returned as
+ * by hicr_fence. */
+int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64_t recv);
+
 /* After hicr_fence returned a deferred error: which batch of that epoch (0-based) and
  * which descriptor index in it was the first bad one.  Host pointers out (may be NULL). */
 int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad);

@@ -37,7 +37,7 @@ assert DESC_DTYPE.itemsize == 32
 EXPORTS = (
     "hicr_init", "hicr_finalize", "hicr_strerror", "hicr_last_cuda_error",
     "hicr_slot_register", "hicr_slot_unregister", "hicr_slot_counters",
-    "hicr_memcpy_batch", "hicr_fence", "hicr_fence_error",
+    "hicr_memcpy_batch", "hicr_fence", "hicr_fence_error", "hicr_fence_async", "hicr_fence_expected",
     "hicr_channel_create", "hicr_channel_destroy", "hicr_channel_counters",
     "hicr_channel_push", "hicr_channel_pop", "hicr_channel_stream",
     "hicr_mpsc_create", "hicr_mpsc_destroy", "hicr_mpsc_counters", "hicr_mpsc_stream",
@@ -64,6 +64,8 @@ def _load() -> ctypes.CDLL:
         "hicr_memcpy_batch": (i32, [vp, vp, u64, i32, P(u64)]),
         "hicr_fence": (i32, [vp]),
         "hicr_fence_error": (i32, [vp, P(u64), P(u64)]),
+        "hicr_fence_async": (i32, [vp]),
+        "hicr_fence_expected": (i32, [vp, u32, u64, u64]),
         "hicr_channel_create": (i32, [vp, u32, u64, u64, P(vp)]),
         "hicr_channel_destroy": (i32, [vp]),
         "hicr_channel_counters": (i32, [vp, P(u64), P(u64)]),
@@ -211,6 +213,18 @@ class Context:
             b, i = ctypes.c_uint64(), ctypes.c_uint64()
             lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
             self._fail(rc, "hicr_fence", first_bad=i.value, batch_index=b.value)
+
+    def fence_async(self):
+        rc = lib.hicr_fence_async(self._h)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_fence_async")
+
+    def fence_expected(self, slot: int, sent: int, recv: int):
+        rc = lib.hicr_fence_expected(self._h, slot, sent, recv)
+        if rc != HICR_OK:
+            b, i = ctypes.c_uint64(), ctypes.c_uint64()
+            lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
+            self._fail(rc, "hicr_fence_expected", first_bad=i.value, batch_index=b.value)
 
     # ---- channels
     def channel_create(self, ring: int, token_bytes: int, capacity: int) -> "Channel":

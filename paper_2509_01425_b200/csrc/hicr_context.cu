@@ -308,6 +308,8 @@ int hicr_slot_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64
     return HICR_OK;
 }
 
+static int close_epoch(hicr_ctx *ctx);
+
 int hicr_fence(hicr_ctx_t *ctx)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
@@ -318,7 +320,13 @@ int hicr_fence(hicr_ctx_t *ctx)
     }
     int rc = drain_epoch(ctx, true);
     if (rc != HICR_OK) return rc;
-    rc = ctx->epoch_error;
+    return close_epoch(ctx);
+}
+
+// Close the epoch as hicr_fence does once everything outstanding has been drained.
+static int close_epoch(hicr_ctx *ctx)
+{
+    const int rc = ctx->epoch_error;
     ctx->last_error = rc;
     ctx->last_error_batch = ctx->epoch_error_batch;
     ctx->last_error_index = ctx->epoch_error_index;
@@ -326,6 +334,61 @@ int hicr_fence(hicr_ctx_t *ctx)
     ctx->epoch_batch_base = 0;
     ctx->epoch_open = false;
     return rc;
+}
+
+int hicr_fence_async(hicr_ctx_t *ctx)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    // Batches are kernels on one stream: each starts after the one before it has completed, so
+    // the ordering the fence promises holds already; only the bookkeeping of completion records,
+    // deferred errors and counters is left open until the next blocking fence.
+    return HICR_OK;
+}
+
+int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64_t recv)
+{
+    if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
+    auto reached = [&] { return ctx->sent[slot] >= sent && ctx->recv[slot] >= recv; };
+    if (reached()) return HICR_OK;
+    if (!ctx->epoch_open || ctx->batches_in_epoch == 0) return HICR_ERR_INVALID_ARG;   // nothing outstanding: never
+    if (slot < kPushSlots && ctx->slots.size() <= kPushSlots) {
+        // Every batch pushes the cumulative counters next to its completion record when its
+        // copies are complete and visible: four flagged words per slot.  A snapshot whose four
+        // flags agree comes from one batch; counters only grow, so the first such snapshot that
+        // reaches the expected counts ends the wait.
+        const unsigned long long *w = ctx->h_rec[kRecRing].w + (size_t)slot * kPushWordsPerSlot;
+        const unsigned long long *last = ctx->h_rec[ctx->batches_in_epoch - 1].w;
+        const uint32_t last_flag = rec_flag(ctx->batch_seq);
+        unsigned spins = 0;
+        for (;;) {
+            uint32_t lf = 0;
+            const bool last_done = word_ready(last + kRwUsed - 1, last_flag, &lf) && word_ready(last, last_flag, &lf);
+            unsigned long long v[kPushWordsPerSlot];
+            for (int k = 0; k < kPushWordsPerSlot; k++) v[k] = *reinterpret_cast<const volatile unsigned long long *>(w + k);
+            const uint32_t f = (uint32_t)(v[0] >> 32);
+            if (f != 0 && (uint32_t)(v[1] >> 32) == f && (uint32_t)(v[2] >> 32) == f && (uint32_t)(v[3] >> 32) == f) {
+                const uint64_t sv = join64((uint32_t)v[0], (uint32_t)v[1]), rv = join64((uint32_t)v[2], (uint32_t)v[3]);
+                if (sv >= ctx->sent[slot] && rv >= ctx->recv[slot]) {
+                    ctx->sent[slot] = sv;
+                    ctx->recv[slot] = rv;
+                }
+                if (reached()) return HICR_OK;
+            }
+            if (last_done) break;   // everything enqueued has completed; look once more below
+            if ((++spins & 0x3fff) == 0) {
+                cudaError_t e = cudaStreamQuery(ctx->stream);
+                if (e != cudaSuccess && e != cudaErrorNotReady) return cuda_fail(ctx, e, "cudaStreamQuery(fence_expected)");
+            }
+        }
+    }
+    // all outstanding work has completed (or the table is too large for pushed counters): an
+    // ordinary fence, after which the counts either are there or never will be
+    int rc = drain_epoch(ctx, true);
+    if (rc != HICR_OK) return rc;
+    rc = close_epoch(ctx);
+    if (rc != HICR_OK) return rc;
+    return reached() ? HICR_OK : HICR_ERR_INVALID_ARG;
 }
 
 int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad)

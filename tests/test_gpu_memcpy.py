@@ -394,3 +394,63 @@ def test_config3a_full_size(hicr):
             o.close()
         sent = np.bincount(d["src_slot"], minlength=n_slots)
         assert [c[0] for c in got_cnt] == sent.tolist()
+
+
+# ------------------------------------------------------------ stream-ordered and expected-count fences
+def test_fence_async_chain(hicr):
+    """hicr_fence_async: config 4's dependency chain with stream-ordered
+    fences between the epochs and one blocking fence at the end leaves the image and the
+    counters the oracle reaches with a blocking fence per epoch."""
+    w = W.chained_epochs(n_epochs=8, n_desc=20000, slot_bytes=32 * W.MiB)
+    ref_imgs, ref_cnt = run_oracle(w)
+    with _ctx(hicr) as ctx:
+        buf = torch.from_numpy(w.slot_image(0)).cuda()
+        sid = ctx.slot_register(buf)
+        keep = []
+        for e in w.epochs:
+            keep.append(to_device_table(e))
+            ctx.memcpy_batch(keep[-1], n=len(e))
+            ctx.fence_async()
+        ctx.fence()
+        assert buf.cpu().numpy().tobytes() == ref_imgs[0].tobytes()
+        assert ctx.slot_counters(sid) == ref_cnt[-1][0] == (8 * 20000, 8 * 20000)
+
+
+def test_fence_expected(hicr):
+    """hicr_fence_expected ("until the expected number of incoming and outgoing data
+    transfers have been completed"): returns once the slot's cumulative counts are reached,
+    reports INVALID_ARG when the enqueued work can never reach them, and leaves the epoch
+    to an ordinary fence.  Reading of DESIGN.md S2 (unpinned by the paper)."""
+    w = W.tiny(n_desc=600, slot_bytes=256 * 1024, max_size=300)
+    parts = np.array_split(w.epochs[0], 3)
+    ref = run_oracle(w)
+    with _ctx(hicr) as ctx:
+        bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(2)]
+        ids = [ctx.slot_register(b) for b in bufs]
+        assert ctx.fence_expected(ids[1], 0, 0) is None                       # already true, nothing outstanding
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence_expected(ids[1], 0, 1)                                  # nothing outstanding: never
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        keep = [to_device_table(p) for p in parts]
+        for t, p in zip(keep, parts):
+            ctx.memcpy_batch(t, n=len(p))
+        ctx.fence_expected(ids[1], 0, len(parts[0]))                          # at least the first batch is in
+        assert ctx.slot_counters(ids[1])[1] >= len(parts[0])
+        ctx.fence_expected(ids[1], 0, 600)
+        ctx.fence_expected(ids[0], 600, 0)
+        assert ctx.slot_counters(ids[1]) == (0, 600) and ctx.slot_counters(ids[0]) == (600, 0)
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == ref[0][s].tobytes()
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence_expected(ids[1], 0, 601)                                # everything is complete: never
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        ctx.fence()
+        # a rejected device batch counts nothing: the expected fence returns its deferred error
+        bad = parts[0].copy()
+        bad["src_slot"][5] = 99
+        t = to_device_table(bad)
+        ctx.memcpy_batch(t, n=len(bad))
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence_expected(ids[1], 0, 600 + len(bad))
+        assert e.value.status == hicr.HICR_ERR_INVALID_SLOT and e.value.first_bad == 5
+        assert ctx.slot_counters(ids[1]) == (0, 600)
