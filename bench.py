@@ -407,6 +407,8 @@ CHANNEL_TEXT = {
     "spsc_calls": "config 5a SPSC, host-call path: push(b_i) then pop(max = capacity), one launch per call",
     "mpsc": "config 5b non-locking MPSC: 148 producers (one CTA per SM), 64 B tokens, 2^20 tokens each, rings of 1024, "
             "single consumer CTA",
+    "mpsc_locking": "config 5b's shape in the paper's LOCKING mode (SURVEY.md S8(f) 2): 148 producers share ONE ring of 1024 "
+                    "tokens of 64 B through atomic reservation and in-order commit, 2^20 tokens each, single consumer CTA",
 }
 
 
@@ -496,7 +498,7 @@ def run_channel(args):
     torch.cuda.set_device(0)
     K, Wm = args.steps, max(1, args.warmup)
     name = args.config
-    if name == "mpsc":
+    if name in ("mpsc", "mpsc_locking"):
         w = W.mpsc() if args.tokens is None else W.mpsc(n_tokens=args.tokens)
     else:
         w = W.spsc() if args.tokens is None else W.spsc(n_tokens=args.tokens)
@@ -504,14 +506,23 @@ def run_channel(args):
     stream = torch.cuda.Stream()
     with torch.cuda.stream(stream):
         ctx = hicr.Context(0, stream.cuda_stream)
-        rings = [torch.zeros(T * C, dtype=torch.uint8, device="cuda") for _ in range(P)]
-        srcs = [torch.from_numpy(w.source_image(p)).cuda() for p in range(P)]
-        sinks = [torch.zeros(N * T, dtype=torch.uint8, device="cuda") for _ in range(P)]
+        locking = name == "mpsc_locking"
+        rings = [torch.zeros(T * C, dtype=torch.uint8, device="cuda") for _ in range(1 if locking else P)]
+        if locking:
+            srcs = [torch.from_numpy(a).cuda() for a in W.generators.tagged_sources(P, N, T)]
+            sinks = [torch.zeros(P * N * T, dtype=torch.uint8, device="cuda")]
+        else:
+            srcs = [torch.from_numpy(w.source_image(p)).cuda() for p in range(P)]
+            sinks = [torch.zeros(N * T, dtype=torch.uint8, device="cuda") for _ in range(P)]
         rid = [ctx.slot_register(t) for t in rings]
         sid = [ctx.slot_register(t) for t in srcs]
         kid = [ctx.slot_register(t) for t in sinks]
         stream.synchronize()
-        if name == "mpsc":
+        if locking:
+            ch = ctx.channel_create(rid[0], T, C)
+            def step():
+                ch.locking_stream(sid, kid[0], 0, N, 256)
+        elif name == "mpsc":
             m = ctx.mpsc_create(rid, T, C)
             def step():
                 m.stream(sid, kid, N, 256)
@@ -547,7 +558,18 @@ def run_channel(args):
         clk = clocks.stop()
         launches = ctx.launch_count() - l0
         ms = e0.elapsed_time(e1)
-        ok = all(torch.equal(a, b) for a, b in zip(srcs, sinks))
+        if locking:
+            # the interleaving is not defined: per-producer FIFO and "every token once", from the tags
+            tags = sinks[0].view(torch.int32).view(P * N, T // 4)[:, :2]
+            order = torch.sort(tags[:, 0].to(torch.int64), stable=True).indices
+            key = tags[order, 0].to(torch.int64) * N + tags[order, 1].to(torch.int64)
+            ok = bool(torch.equal(key, torch.arange(P * N, device="cuda")))
+            del key, tags
+            allsrc = torch.cat(srcs).view(P * N, T)
+            ok = ok and bool(torch.equal(sinks[0].view(P * N, T)[order], allsrc))
+            del allsrc, order
+        else:
+            ok = all(torch.equal(a, b) for a, b in zip(srcs, sinks))
     tokens = float(P) * N
     bytes_step = 4.0 * tokens * T
     peak, peak_src = load_peaks()
@@ -563,7 +585,7 @@ def run_channel(args):
                 "d2h_bytes_per_step": 32 * (2 * len(w.batches[0]) if name == "spsc_calls" else 1),
                 "ms_per_step": 1e3 * t_host / K, "what": "host wall clock around the blocking calls"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": "spsc_stream_kernel" if name != "mpsc" else "mpsc_stream_kernel",
+        "roofline": {"bound": "hbm", "kernel": {"mpsc": "mpsc_stream_kernel", "mpsc_locking": "mpsc_locking_kernel"}.get(name, "spsc_stream_kernel"),
                      "achieved": gbs / 2, "peak": peak, "unit": UNIT, "frac": gbs / 2 / peak, "traffic": None,
                      "peak_source": peak_src,
                      "note": "DRAM sees source and sink only (the ring lives in L2): algorithmic DRAM bytes = 2 x payload; "

@@ -221,6 +221,21 @@ int hicr_mpsc_counters(hicr_mpsc_t *m, uint32_t producer, uint64_t *head, uint64
 int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_slot_t *dst_slots,
                      uint64_t tokens_per_producer, uint64_t max_batch);
 
+/* Device-resident LOCKING MPSC run ("locking, where a collective exclusive
+ * access guarantees a shared channel does not overflow"): `producers` producer CTAs push
+ * tokens_per_producer tokens each, from src_slots[p] (offset 0), into the ONE ring of the
+ * SPSC channel `ch`, in batches of at most max_batch tokens; a single consumer CTA pops them
+ * into `dst`, consecutively from dst_off, in the order they entered the ring.  The
+ * exclusive access is an atomic reservation of ring positions that succeeds only while the
+ * positions are free, followed by a commit in reservation order.  The interleaving of
+ * producers in `dst` is not defined; what is: each producer's tokens appear in its own
+ * order (per-producer FIFO), every token exactly once, head = tail advanced by
+ * producers * tokens_per_producer, one message per token on every slot.  Requires an empty
+ * ring at entry and all producers + 1 CTAs co-resident (HICR_ERR_NO_CAPACITY otherwise).
+ * src_slots: host pointer to `producers` ids.  Blocks until done. */
+int hicr_mpsc_locking_stream(hicr_channel_t *ch, uint32_t producers, const hicr_slot_t *src_slots, hicr_slot_t dst,
+                             uint64_t dst_off, uint64_t tokens_per_producer, uint64_t max_batch);
+
 /* ---- measurement hooks (plumbing) -------------------------------------------------- */
 
 /* Kernel launches issued by this context since hicr_init (host pointer out). */

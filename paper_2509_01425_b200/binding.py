@@ -41,6 +41,7 @@ EXPORTS = (
     "hicr_channel_create", "hicr_channel_destroy", "hicr_channel_counters",
     "hicr_channel_push", "hicr_channel_pop", "hicr_channel_stream",
     "hicr_mpsc_create", "hicr_mpsc_destroy", "hicr_mpsc_counters", "hicr_mpsc_stream",
+    "hicr_mpsc_locking_stream",
     "hicr_launch_count", "hicr_profile_enable", "hicr_profile_read",
 )
 
@@ -76,6 +77,7 @@ def _load() -> ctypes.CDLL:
         "hicr_mpsc_destroy": (i32, [vp]),
         "hicr_mpsc_counters": (i32, [vp, u32, P(u64), P(u64)]),
         "hicr_mpsc_stream": (i32, [vp, vp, vp, u64, u64]),
+        "hicr_mpsc_locking_stream": (i32, [vp, u32, vp, u32, u64, u64, u64]),
         "hicr_launch_count": (i32, [vp, P(u64)]),
         "hicr_profile_enable": (i32, [vp, i32]),
         "hicr_profile_read": (i32, [vp, P(ctypes.c_float)]),
@@ -301,6 +303,14 @@ class Channel:
         if rc != HICR_OK:
             self._ctx._fail(rc, "hicr_channel_pop")
         return k.value
+
+    def locking_stream(self, src_slots, dst: int, dst_off: int, tokens_per_producer: int, max_batch: int):
+        """hicr_mpsc_locking_stream: len(src_slots) producers share this channel's ring."""
+        ids = _slot_ids(src_slots)
+        rc = lib.hicr_mpsc_locking_stream(self._h, ids.size, ctypes.c_void_p(ids.ctypes.data), dst, dst_off,
+                                          tokens_per_producer, max_batch)
+        if rc != HICR_OK:
+            self._ctx._fail(rc, "hicr_mpsc_locking_stream")
 
     def stream(self, src: int, src_off: int, dst: int, dst_off: int, batch_tokens):
         b = np.ascontiguousarray(np.asarray(batch_tokens, dtype=np.uint64))

@@ -340,6 +340,93 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
     if (use_tma && lane == 0) bulk_wait_all();   // the sink is complete (and shared memory free) before the CTA exits
 }
 
+// Device-resident LOCKING MPSC run ("locking, where a collective exclusive access
+// guarantees a shared channel does not overflow"): P producer CTAs share ONE ring.  The
+// exclusive access is an atomic reservation: a producer advances `reserve` by k only if the k
+// positions are free (reserve + k - tail <= C, compare-and-swap), copies its tokens into the
+// positions it owns, and commits in reservation order -- it waits until head has reached its
+// first position and then moves head past its last one.  Each wait is on a producer that
+// reserved earlier and is co-resident (cooperative launch), so the chain always advances.
+// CTA P is the single consumer: pops whatever head shows into dst, consecutively.
+// srcs = source base addresses x P; slot_ids = source slot ids x P (message counters).
+__global__ void __launch_bounds__(kMpscThreads, 2)
+mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, unsigned char *ring, uint64_t T,
+                    uint64_t C, const uint64_t *__restrict__ srcs, const uint32_t *__restrict__ slot_ids,
+                    unsigned char *dst, uint64_t tokens, uint64_t max_batch, unsigned long long *sent,
+                    unsigned long long *recv, uint32_t ring_slot, uint32_t dst_slot, CallResult *res)
+{
+    __shared__ unsigned long long sh_start, sh_k;
+    const uint64_t ring_bytes = C * T;
+    const int tid = threadIdx.x;
+    if (blockIdx.x < P) {
+        const uint32_t p = blockIdx.x;
+        unsigned char *src = reinterpret_cast<unsigned char *>(srcs[p]);
+        uint64_t pushed = 0;
+        while (pushed < tokens) {
+            if (tid == 0) {
+                const unsigned long long want = min((unsigned long long)(tokens - pushed), (unsigned long long)max_batch);
+                unsigned ns = 20;
+                for (;;) {
+                    const unsigned long long r = *reinterpret_cast<volatile unsigned long long *>(reserve);
+                    const unsigned long long room = C - (r - ld_acquire(&st->tail));   // tail <= head <= reserve
+                    if (room == 0 || room > C) {   // full (or a tail newer than the reserve value just read)
+                        backoff(ns);
+                        continue;
+                    }
+                    const unsigned long long k = min(want, room);
+                    if (atomicCAS(reserve, r, r + k) == r) {
+                        sh_start = r;
+                        sh_k = k;
+                        break;
+                    }
+                }
+            }
+            __syncthreads();
+            const uint64_t start = sh_start, k = sh_k;
+            ring_copy<2, true>(ring, ring_bytes, (start % C) * T, src + pushed * T, k * T, tid, kMpscThreads);
+            __syncthreads();
+            if (tid == 0) {
+                unsigned ns = 20;
+                while (ld_acquire(&st->head) != start) backoff(ns);   // commit in reservation order
+                st_release(&st->head, start + k);
+            }
+            pushed += k;
+        }
+        if (tid == 0) atomicAdd(&sent[slot_ids[p]], (unsigned long long)tokens);
+        return;
+    }
+    // ---- the single consumer
+    const uint64_t total = (uint64_t)P * tokens;
+    unsigned long long tail = st->tail;
+    const unsigned long long tail0 = tail;
+    uint64_t popped = 0;
+    while (popped < total) {
+        if (tid == 0) {
+            unsigned ns = 20;
+            unsigned long long avail;
+            while ((avail = ld_acquire(&st->head) - tail) == 0) backoff(ns);
+            sh_k = avail;
+        }
+        __syncthreads();
+        const uint64_t k = sh_k;
+        ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + popped * T, k * T, tid, kMpscThreads);
+        __syncthreads();
+        if (tid == 0) st_release(&st->tail, tail + k);
+        tail += k;
+        popped += k;
+    }
+    if (tid == 0) {
+        atomicAdd(&recv[ring_slot], (unsigned long long)total);
+        atomicAdd(&sent[ring_slot], (unsigned long long)total);
+        atomicAdd(&recv[dst_slot], (unsigned long long)total);
+        res->k = total;
+        res->head = tail0 + total;
+        res->tail = tail;
+        res->status = HICR_OK;
+        __threadfence_system();
+    }
+}
+
 // The kernel wrote the result into mapped pinned memory before the stream synchronize returned.
 static CallResult read_result(hicr_ctx *ctx)
 {
@@ -657,6 +744,74 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_sl
         ctx->sent[m->rings[p]] += N;
         ctx->recv[dst_slots[p]] += N;
     }
+    return HICR_OK;
+}
+
+int hicr_mpsc_locking_stream(hicr_channel_t *ch, uint32_t producers, const hicr_slot_t *src_slots, hicr_slot_t dst,
+                             uint64_t dst_off, uint64_t tokens_per_producer, uint64_t max_batch)
+{
+    if (!ch || !src_slots || producers == 0 || max_batch == 0) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = ch->ctx;
+    const uint32_t P = producers;
+    const uint64_t N = tokens_per_producer;
+    if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;   // requires an empty ring at entry
+    if (!slot_ok(ctx, dst)) return HICR_ERR_INVALID_SLOT;
+    if (N > (1ull << 48) / ch->T / P) return HICR_ERR_OUT_OF_BOUNDS;
+    for (uint32_t p = 0; p < P; p++) {
+        if (!slot_ok(ctx, src_slots[p])) return HICR_ERR_INVALID_SLOT;
+        if (N * ch->T > ctx->slots[src_slots[p]].size) return HICR_ERR_OUT_OF_BOUNDS;
+    }
+    const SlotRow &ds = ctx->slots[dst];
+    if (dst_off > ds.size || (uint64_t)P * N * ch->T > ds.size - dst_off) return HICR_ERR_OUT_OF_BOUNDS;
+    if (N == 0) return HICR_OK;
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    // co-residency of all P + 1 CTAs is what makes the spin-waits (reservation, in-order commit) safe
+    int per_sm = 0;
+    HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_locking_kernel, kMpscThreads, 0));
+    if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
+
+    std::vector<uint64_t> ptrs(P);
+    std::vector<uint32_t> ids(P);
+    for (uint32_t p = 0; p < P; p++) {
+        ptrs[p] = ctx->slots[src_slots[p]].base;
+        ids[p] = src_slots[p];
+    }
+    unsigned char *d_tab = nullptr;   // [P] u64 source bases, [P] u32 slot ids, one u64 reservation counter
+    const size_t tab_bytes = (size_t)P * 12 + 16;
+    HICR_CUDA(ctx, cudaMalloc(&d_tab, tab_bytes));
+    uint64_t *d_ptrs = reinterpret_cast<uint64_t *>(d_tab);
+    unsigned long long *d_reserve = reinterpret_cast<unsigned long long *>(d_tab + (size_t)P * 8);
+    uint32_t *d_ids = reinterpret_cast<uint32_t *>(d_tab + (size_t)P * 8 + 8);
+    const unsigned long long head0 = ch->head;
+    cudaError_t e = cudaMemcpyAsync(d_ptrs, ptrs.data(), (size_t)P * 8, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_reserve, &head0, 8, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(d_ids, ids.data(), (size_t)P * 4, cudaMemcpyHostToDevice, ctx->stream);
+    if (e == cudaSuccess) {
+        ChannelState *st = ch->d_state;
+        uint32_t Pv = P, ring_slot = ch->ring, dst_slot = dst;
+        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+        unsigned char *dp = reinterpret_cast<unsigned char *>(ds.base + dst_off);
+        uint64_t T = ch->T, C = ch->C, tok = N, mb = max_batch;
+        const uint64_t *pp = d_ptrs;
+        const uint32_t *ip = d_ids;
+        unsigned long long *sent = ctx->d_sent, *recv = ctx->d_recv;
+        CallResult *res = ctx->d_call;
+        void *args[] = {&st, &d_reserve, &Pv, &ring, &T, &C, &pp, &ip, &dp, &tok, &mb, &sent, &recv, &ring_slot, &dst_slot, &res};
+        e = cudaLaunchCooperativeKernel((const void *)mpsc_locking_kernel, dim3(P + 1), dim3(kMpscThreads), args, 0,
+                                        ctx->stream);
+        ctx->launches++;
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+    cudaFree(d_tab);
+    if (e != cudaSuccess) return cuda_fail(ctx, e, "hicr_mpsc_locking_stream");
+    const CallResult r = read_result(ctx);
+    ch->head = r.head;
+    ch->tail = r.tail;
+    const uint64_t total = (uint64_t)P * N;
+    for (uint32_t p = 0; p < P; p++) ctx->sent[src_slots[p]] += N;
+    ctx->recv[ch->ring] += total;
+    ctx->sent[ch->ring] += total;
+    ctx->recv[dst] += total;
     return HICR_OK;
 }
 

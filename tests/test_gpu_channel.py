@@ -338,3 +338,68 @@ def test_pingpong_capacity_one(hicr, s):
         assert imgs[3].tobytes() == imgs[2].tobytes()
         for i in ids:
             assert ctx.slot_counters(i) == o.slot_counters(i)
+
+
+# ------------------------------------------------------------ locking MPSC
+def _check_locking_sink(sink, srcs, T):
+    """Invariants of a locking MPSC run, from the sink alone: every token is some producer's
+    token (byte for byte), each producer's tokens appear in its own order, every token once."""
+    P, N = len(srcs), srcs[0].size // T
+    tok = sink.reshape(P * N, T)
+    tag = np.ascontiguousarray(tok[:, :8]).view("<u4").reshape(P * N, 2)
+    prod, idx = tag[:, 0].astype(np.int64), tag[:, 1].astype(np.int64)
+    assert prod.min() >= 0 and prod.max() < P
+    for p in range(P):
+        mine = np.nonzero(prod == p)[0]
+        assert mine.size == N, "producer %d: %d tokens in the sink" % (p, mine.size)
+        assert np.array_equal(idx[mine], np.arange(N)), "producer %d out of order" % p       # FIFO, each once
+        assert np.array_equal(tok[mine], srcs[p].reshape(N, T)), "producer %d payload" % p
+
+
+@pytest.mark.timeout(600)
+@pytest.mark.parametrize("P,N,T,C,maxb", [(1, 4000, 16, 8, 5), (4, 3000, 24, 16, 7), (37, 2000, 64, 64, 48),
+                                          (148, 4096, 64, 1024, 256), (9, 500, 100, 1, 3)])
+def test_mpsc_locking(hicr, P, N, T, C, maxb):
+    """Locking MPSC: P producers share one ring through atomic reservation and
+    in-order commit.  The interleaving is not defined, so the result is checked by its
+    invariants; the same checker accepts the oracle's run of a seeded interleaving on one
+    shared channel (sequential pushes = exclusive access), and head, tail and all message
+    counters agree with it."""
+    srcs = W.generators.tagged_sources(P, N, T)
+    # oracle: one channel, producers take turns in a seeded order, consumer drains after each push
+    o = Oracle()
+    ring, sink = np.zeros(T * C, np.uint8), np.zeros(P * N * T, np.uint8)
+    rid = o.slot_register(ring)
+    sid = [o.slot_register(a.copy()) for a in srcs]
+    kid = o.slot_register(sink)
+    _, och = o.channel_create(rid, T, C)
+    rng = np.random.default_rng(P * 1000 + C)
+    left, pushed, popped = [N] * P, [0] * P, 0
+    while any(left):
+        p = int(rng.choice([q for q in range(P) if left[q]]))
+        rc, k = o.channel_push(och, sid[p], pushed[p] * T, min(left[p], int(rng.integers(1, maxb + 1))))
+        assert rc == oracle.OK and k > 0
+        pushed[p] += k
+        left[p] -= k
+        rc, k2 = o.channel_pop(och, kid, popped * T, C)
+        assert k2 == k
+        popped += k
+    _check_locking_sink(sink, srcs, T)
+
+    with _ctx(hicr) as ctx:
+        g_ring = torch.zeros(T * C, dtype=torch.uint8, device="cuda")
+        g_src = [torch.from_numpy(a).cuda() for a in srcs]
+        g_sink = torch.zeros(P * N * T, dtype=torch.uint8, device="cuda")
+        assert ctx.slot_register(g_ring) == rid
+        assert [ctx.slot_register(t) for t in g_src] == sid
+        assert ctx.slot_register(g_sink) == kid
+        ch = ctx.channel_create(rid, T, C)
+        ch.locking_stream(sid, kid, 0, N, maxb)
+        torch.cuda.synchronize()
+        _check_locking_sink(g_sink.cpu().numpy(), srcs, T)
+        assert ch.counters() == o.channel_counters(och) == (P * N, P * N)
+        for s in [rid, kid] + sid:
+            assert ctx.slot_counters(s) == o.slot_counters(s)
+        # the channel keeps working through host calls afterwards, on the same counters
+        assert ch.push(sid[0], 0, 1) == 1 and ch.pop(kid, 0, 1) == 1
+        assert ch.counters() == (P * N + 1, P * N + 1)

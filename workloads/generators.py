@@ -283,3 +283,21 @@ def mpsc(producers: int = 148, n_tokens: int = 1 << 20, token_bytes: int = 64, c
     sched = np.concatenate([np.full(len(b), p, dtype=np.int64) for p, b in enumerate(batches)])
     rng.shuffle(sched)
     return ChannelWorkload("mpsc", producers, token_bytes, capacity, n_tokens, batches, sched, seed)
+
+
+def tagged_sources(producers: int, n_tokens: int, token_bytes: int, seed: int = BASE_SEED):
+    """Sources for the LOCKING MPSC run, whose interleaving in the sink is
+    not defined: token i of producer p is random bytes with a tag in its first 8 bytes --
+    little-endian u32 p, u32 i -- so that a checker can recover, from the sink alone, which
+    producer's which token sits where (per-producer order, every token exactly once)."""
+    if token_bytes < 8:
+        raise ValueError("tagged tokens need at least 8 bytes")
+    out = []
+    for p in range(producers):
+        a = random_bytes(rng_for(5, 2000 + p, seed), n_tokens * token_bytes).reshape(n_tokens, token_bytes)
+        tag = np.empty((n_tokens, 2), dtype="<u4")
+        tag[:, 0] = p
+        tag[:, 1] = np.arange(n_tokens, dtype=np.uint32)
+        a[:, :8] = tag.view(np.uint8).reshape(n_tokens, 8)
+        out.append(np.ascontiguousarray(a.reshape(-1)))
+    return out
