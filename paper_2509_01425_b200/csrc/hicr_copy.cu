@@ -9,22 +9,24 @@
 //
 // engine_kernel, grid = SMs x kCtasPerSm co-resident CTAs of 256 threads:
 //   phase A  one thread per descriptor (grid-stride tiles): validate against the slot
-//            table, resolve absolute addresses, classify by size, compact into the warp
-//            queue / expand into the chunk queue (warp ballot + warp prefix sums + one
-//            atomic per warp per queue), count messages per slot in a shared-memory
-//            histogram.
-//   barrier  grid-wide, ONE 64-bit word: arrivals, "saw an invalid descriptor" votes and the
-//            chunk-queue length share it, so the poll that sees the last arrival also
-//            delivers the verdict.  Any invalid descriptor: nothing is copied or counted
-//            (all-or-nothing).  While the barrier fills, every warp prefetches the sources
-//            of its first descriptors into L2.
+//            table, resolve absolute addresses, expand descriptors above 8 KiB into the chunk
+//            queue (warp ballot + warp prefix sum + one atomic per warp), count messages per
+//            slot in a shared-memory histogram; small descriptors stay in the table.
+//   barrier  grid-wide, ONE 64-bit word: arrivals, "saw an invalid descriptor" votes, "my small
+//            descriptors are team-sized" votes and the chunk-queue length share it, so the
+//            poll that sees the last arrival also delivers the verdict.  Any invalid
+//            descriptor: nothing is copied or counted (all-or-nothing).  While the barrier
+//            fills, every warp prefetches the sources of its first descriptors into L2.
+//            Host-validated tables without large descriptors skip the barrier.
 //   phase B  histogram flushed into the cumulative u64 counters (one atomic per touched
-//            slot per CTA); then dynamic work tickets (one atomic per CTA per ticket,
-//            prefetched one round ahead): a ticket is one chunk (CTA-per-chunk) or eight
-//            small descriptors (warp-per-descriptor).  16 B-aligned spans of at least
-//            tma_min bytes go through 1-D TMA bulk copies staged in shared memory, one
-//            4 KiB stage per warp; everything else through 16 B vector loads / aligned
-//            stores with byte-shifted sources (copy_span).
+//            slot per CTA).  B1, CTA per 128 KiB chunk: dynamic tickets, thread 0 two rounds
+//            ahead (next item loaded, ticket after that in flight); 16 B-aligned chunks go
+//            through 1-D TMA bulk copies staged in shared memory, the rest through 16 B vector
+//            loads / aligned stores with byte-shifted sources (copy_span).  B2, small
+//            descriptors read from the table in place: warp tickets by guided self-scheduling
+//            (three in flight per warp), or equal static shares when the batch is team-sized;
+//            > 256 B: copy_span by the warp; <= 256 B: copy_team, eight descriptors at a time
+//            by teams of four lanes, every load before the first store.
 //   finish   the last CTA to finish pushes the counters and the completion record into
 //            mapped pinned host memory (what hicr_fence polls) and clears the control block.
 #include "hicr_internal.cuh"
