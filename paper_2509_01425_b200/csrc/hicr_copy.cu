@@ -379,8 +379,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         // host-validated table without large descriptors: nothing to agree on, nothing to wait for
         __syncthreads();
     } else {
+        // only CTAs that validated a tile have anything to say: the others wait for the verdict
+        // without arriving (a 256-descriptor batch is a barrier of one arrival, not 296)
+        const unsigned arrivals = min((unsigned)gridDim.x, (n + kThreads - 1) / kThreads);
         const int cta_bad = __syncthreads_or(bad_seen);
-        if (tid == 0) {
+        if (tid == 0 && blockIdx.x < arrivals) {
             const unsigned long long vote = sh_small[1] != 0 && sh_small[0] <= (unsigned long long)(kTeamMax / 16) * sh_small[1];
             atom_add_release_u64(&ctl->sync, 1ull | ((unsigned long long)(cta_bad != 0) << kSyncBadShift) |
                                                  (vote << kSyncVoteShift));
@@ -399,7 +402,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         }
         if (tid == 0) {
             unsigned long long v;
-            while (((v = ld_acquire(&ctl->sync)) & kSyncFieldMask) < gridDim.x) {}
+            while (((v = ld_acquire(&ctl->sync)) & kSyncFieldMask) < arrivals) {}
             sh_sync = v;
         }
         __syncthreads();
