@@ -486,6 +486,34 @@ def run_pingpong(args):
     return 0
 
 
+def oracle_channel_sample(w, budget_s: float):
+    """cpu_baseline of the channel configs: the oracle's push / pop(max = C) loop, token by token,
+    on ONE ring (producer 0's batches and source prefix), until ``budget_s`` of CPU time."""
+    from oracle import Oracle
+    T, C = w.token_bytes, w.capacity
+    batches = w.batches[0]
+    n_cap = int(min(w.n_tokens, 1 << 22))                       # at most 2^22 tokens of the source prefix
+    src = np.random.default_rng(w.seed).integers(0, 256, n_cap * T, dtype=np.uint8)   # timing only: any bytes do
+    ring, sink = np.zeros(T * C, np.uint8), np.zeros(n_cap * T, np.uint8)
+    o = Oracle()
+    r, s, k = o.slot_register(ring), o.slot_register(src), o.slot_register(sink)
+    _, ch = o.channel_create(r, T, C)
+    pos, nb = 0, 0
+    t0 = time.perf_counter()
+    for b in batches:
+        b = int(b)
+        if pos + b > n_cap or time.perf_counter() - t0 > budget_s:
+            break
+        o.channel_push(ch, s, pos * T, b)
+        o.channel_pop(ch, k, pos * T, C)
+        pos += b
+        nb += 1
+    dt = time.perf_counter() - t0
+    return {"value": 4.0 * pos * T / dt / 1e9, "unit": UNIT, "cores": 1, "kind": "oracle", "tokens_per_s": pos / dt,
+            "sample": "push / pop(max = C) of the first %d batches (%d tokens of %d B) of one ring in %.1f s "
+                      "(host cores available: %d)" % (nb, pos, T, dt, host_cores())}
+
+
 def run_channel(args):
     """Configs 5a / 5b.  A step is the whole push/pop sequence; bytes = 4 x payload (source ->
     ring -> sink, read + write each hop).  value = device time of the sequence; e2e = the
@@ -590,7 +618,8 @@ def run_channel(args):
                      "peak_source": peak_src,
                      "note": "DRAM sees source and sink only (the ring lives in L2): algorithmic DRAM bytes = 2 x payload; "
                              "the bound that binds is one producer CTA and one consumer CTA per ring, not HBM"},
-        "cpu_baseline": None, "clocks": clk, "sink_equals_source": bool(ok),
+        "cpu_baseline": None if args.no_cpu_baseline else oracle_channel_sample(w, args.cpu_seconds),
+        "clocks": clk, "sink_equals_source": bool(ok),
     }
     print(json.dumps(line))
     ctx.close()
