@@ -638,7 +638,7 @@ static int get_stage(hicr_ctx *ctx, size_t bytes, StageBlock *out)
     }
     StageBlock b;
     b.bytes = std::max<size_t>(bytes, 1 << 20);
-    HICR_CUDA(ctx, cudaHostAlloc(&b.host, b.bytes, cudaHostAllocDefault));
+    HICR_CUDA(ctx, cudaHostAlloc(&b.host, b.bytes, cudaHostAllocMapped | cudaHostAllocPortable));
     cudaError_t e = cudaMalloc(&b.dev, b.bytes);
     if (e != cudaSuccess) {
         cudaFreeHost(b.host);
@@ -712,7 +712,8 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         }
         units = nc + (ns + kWarps - 1) / kWarps;
         ctx->used_stage.push_back(b);
-        d_descs = static_cast<const hicr_desc_t *>(b.dev);
+        // pinned staging is device-accessible under unified addressing: short tables stay there
+        d_descs = static_cast<const hicr_desc_t *>(n <= kZeroCopyDescs ? b.host : b.dev);
         // checked against the host mirror of the slot table, which the device copy follows in
         // stream order: with no chunk queue to wait for either, the kernel needs no barrier
         skip_barrier = nc == 0;

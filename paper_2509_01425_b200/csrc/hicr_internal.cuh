@@ -36,6 +36,8 @@ constexpr uint32_t kPushSlots = 256;       // counters of the first kPushSlots s
 constexpr int kTeam = 4;                   // lanes per team
 constexpr int kTeamVecs = 4;               // 16 B vectors per lane of a team
 constexpr unsigned kTeamMax = 16 * kTeam * kTeamVecs;   // descriptors up to this size (256 B) are copied by teams, 32 / kTeam at a time
+constexpr uint64_t kZeroCopyDescs = 1024;   // host tables up to this many descriptors are read by the kernel straight from
+                                            // pinned staging (32 KiB over PCIe costs less than enqueueing a copy: ~1.5 vs ~5 us)
 constexpr unsigned kMaxGroup = 32;         // units per warp ticket, at most (one per lane)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
