@@ -673,6 +673,8 @@ int engine_setup(hicr_ctx *ctx)
     if (e && *e) ctx->gss = (uint32_t)std::max(1, atoi(e));
     e = getenv("HICR_MAX_GROUP");
     if (e && *e) ctx->max_group = (uint32_t)std::max(1, std::min((int)kMaxGroup, atoi(e)));
+    e = getenv("HICR_ZERO_COPY");
+    if (e && *e) ctx->zero_copy_descs = strtoull(e, nullptr, 0);
     e = getenv("HICR_PREFETCH");
     if (e && *e) ctx->prefetch = (uint32_t)std::max(0, std::min(32, atoi(e)));
     ctx->engine_grid = (int)std::min<unsigned>(ctx->num_sms * per_sm, kMaxGrid);
@@ -713,7 +715,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         units = nc + (ns + kWarps - 1) / kWarps;
         ctx->used_stage.push_back(b);
         // pinned staging is device-accessible under unified addressing: short tables stay there
-        d_descs = static_cast<const hicr_desc_t *>(n <= kZeroCopyDescs ? b.host : b.dev);
+        d_descs = static_cast<const hicr_desc_t *>(n <= ctx->zero_copy_descs ? b.host : b.dev);
         // checked against the host mirror of the slot table, which the device copy follows in
         // stream order: with no chunk queue to wait for either, the kernel needs no barrier
         skip_barrier = nc == 0;

@@ -183,7 +183,7 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
             ready++;
         }
         if (rc != HICR_OK) break;
-        if (n <= kZeroCopyDescs) {
+        if (n <= ctx->zero_copy_descs) {
             sent = ready;   // short table: the kernel reads the pinned staging block in place (no copy to enqueue)
         } else if (ready - sent >= kSendPieces || (ready == j.n_pieces && ready > sent)) {
             const uint64_t i0 = sent * kPiece, i1 = std::min(n, ready * kPiece);
