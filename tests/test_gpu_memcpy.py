@@ -454,3 +454,16 @@ def test_fence_expected(hicr):
             ctx.fence_expected(ids[1], 0, 600 + len(bad))
         assert e.value.status == hicr.HICR_ERR_INVALID_SLOT and e.value.first_bad == 5
         assert ctx.slot_counters(ids[1]) == (0, 600)
+
+
+@pytest.mark.timeout(600)
+def test_no_access_past_the_end_of_a_slot():
+    """Slots that end on the last mapped byte before unmapped virtual addresses: a kernel that
+    reads or writes one 16-byte granule too far faults.  Runs in a subprocess (a fault poisons
+    the CUDA context); see tests/guard_page_check.py."""
+    import subprocess
+    import sys
+    r = subprocess.run([sys.executable, os.path.join(os.path.dirname(__file__), "guard_page_check.py")],
+                       capture_output=True, text=True, timeout=550)
+    assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
+    assert "guard page check ok" in r.stdout
