@@ -268,7 +268,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
     const unsigned gdiv = a.gss * nw, gmax = a.max_group;
     auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, 1u), gmax); };
-    const unsigned cnt_static = ticket_size(n, 0), static_end = nw * cnt_static;
+    // (a multiple of 8 when it can be: team-sized descriptors are copied 8 at a time)
+    const unsigned cnt_static0 = ticket_size(n, 0), cnt_static = cnt_static0 >= 8 ? cnt_static0 & ~7u : cnt_static0;
+    const unsigned static_end = nw * cnt_static;
     __syncthreads();
 
     // ================================================================ phase A (a2, a3, a6)
