@@ -25,7 +25,7 @@ constexpr int kWarps = kThreads / 32;
 constexpr int kCtasPerSm = 2;              // persistent grid = SMs x kCtasPerSm; 16 warps x 4 x 16 B x 32 lanes = 32 KiB of
                                            // loads in flight per SM is where a 4 KiB page copy peaks on B200 (S5)
 constexpr int kUnroll = 4;                 // 16-byte vectors in flight per lane (aligned source)
-constexpr int kUnrollShifted = 4;          // the same for byte-shifted sources
+constexpr int kUnrollShifted = 8;          // the same for byte-shifted sources
 constexpr uint32_t kSmemSlotHist = 1024;   // per-CTA shared-memory counter histogram up to this many slots
 constexpr uint32_t kSlotCache = 256;       // slot-table rows cached in shared memory (larger tables are read from L2)
 constexpr uint32_t kTmaPiece = 4096;       // bytes per bulk copy
