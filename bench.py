@@ -235,6 +235,18 @@ def load_peaks():
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
+def pin_rate_gbs(device: int = 0):
+    """Memory clock x 2 x bus width / 8 from the device properties (3996 MHz x 2 x 7680 bit / 8 =
+    7672 GB/s on B200): the second denominator of SURVEY.md S8(d).  The measured peak is a
+    torch copy calibration, not a ceiling: long streaming copies of this engine exceed it."""
+    try:
+        import torch
+        p = torch.cuda.get_device_properties(device)
+        return float(p.memory_clock_rate) * 1e3 * 2.0 * float(p.memory_bus_width) / 8.0 / 1e9
+    except Exception:
+        return None
+
+
 def run_cuda(args):
     import torch
     import paper_2509_01425_b200 as hicr
@@ -347,6 +359,7 @@ def run_cuda(args):
 
     if rank == 0:
         peak, peak_src = load_peaks()
+        pin = pin_rate_gbs(local)
         prof /= max(1, n_prof)
         kernel_ms = {"plan_phase": prof[0], "copy_phase": prof[1], "engine_kernel_globaltimer": prof[2],
                      "engine_kernel": prof[3]}
@@ -388,7 +401,8 @@ def run_cuda(args):
             "kernel_ms": kernel_ms,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": UNIT,
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
-                         "algorithmic_bytes_per_launch": bps},
+                         "algorithmic_bytes_per_launch": bps, "pin_rate": pin,
+                         "frac_of_pin_rate": (achieved / pin) if pin else None},
             "cpu_baseline": cpu,
             "clocks": clk,
             "counters_ok": bool(sum(c[0] for c in counters) == sum(c[1] for c in counters)),
