@@ -467,3 +467,36 @@ def test_no_access_past_the_end_of_a_slot():
                        capture_output=True, text=True, timeout=550)
     assert r.returncode == 0, r.stdout[-2000:] + r.stderr[-4000:]
     assert "guard page check ok" in r.stdout
+
+
+@pytest.mark.timeout(900)
+def test_randomized_mixes(hicr):
+    """60 seeded workloads drawn from all four generators with random sizes of slot, batch and
+    descriptor (team, warp and chunk classes mixed, 1 to 3 batches per epoch), each through
+    host tables and device tables: every byte and counter equals the oracle's."""
+    rng = np.random.default_rng(W.BASE_SEED + 99)
+    done = 0
+    while done < 60:
+        seed, kind = int(rng.integers(1, 1 << 30)), int(rng.integers(0, 4))
+        try:
+            if kind == 0:
+                w = W.heavy_tailed("a", n_slots=int(rng.integers(2, 70)), slot_bytes=int(rng.integers(3, 9)) * W.MiB,
+                                   src_zone=W.MiB, n_desc=int(rng.integers(1, 6000)),
+                                   smax=int(rng.choice([300, 9000, 200000, 900000])), seed=seed)
+            elif kind == 1:
+                w = W.tiny(n_desc=int(rng.integers(1, 3000)), slot_bytes=int(rng.integers(1, 5)) * W.MiB,
+                           max_size=int(rng.choice([16, 256, 300, 4096, 20000])), seed=seed)
+            elif kind == 2:
+                w = W.chained_epochs(n_epochs=int(rng.integers(2, 6)), n_desc=int(rng.integers(10, 30000)),
+                                     slot_bytes=16 * W.MiB, smin=int(rng.choice([1, 8])),
+                                     smax=int(rng.choice([16, 256, 1000])), seed=seed)
+            else:
+                w = W.bulk_aligned(n_desc=int(rng.integers(1, 5000)), slot_bytes=64 * W.MiB,
+                                   page=int(rng.choice([16, 256, 1024, 4096, 16384])), n_sets=2, seed=seed)
+        except ValueError:
+            continue                                   # the draw does not fit its slots
+        ref = run_oracle(w)
+        for dev in (False, True):
+            got = run_gpu(w, device_tables=dev, split=int(rng.integers(1, 4)))
+            assert_same(w, ref, got, "kind %d seed %d device_tables %s" % (kind, seed, dev))
+        done += 1
