@@ -121,7 +121,8 @@ static_assert(sizeof(ChannelState) == 256, "ChannelState is two lines");
 struct CallResult {
     unsigned long long k, head, tail;
     long long status;
-    unsigned long long seq;   // written last, after a system-scope fence: the host polls it (host-call path)
+    unsigned long long seq;   // (unused by the kernels; the host keeps the call's sequence number here)
+    unsigned long long w[8];  // host-call path: the result as flagged words {flag:32 | payload:32}, polled by the host
 };
 
 #ifdef __CUDACC__
