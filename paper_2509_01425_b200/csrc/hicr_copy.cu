@@ -225,6 +225,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     __shared__ WorkItem sh_item[2];              // queue items of the current and the next chunk
     __shared__ unsigned sh_flag;
     __shared__ unsigned long long sh_sync;       // the barrier word as the last poll saw it
+    __shared__ unsigned sh_first1;               // first descriptor of the CTA's second tickets (warp w: + w x cnt1)
     __shared__ unsigned sh_small[2];             // bytes and count of the small descriptors this CTA validated
     __shared__ unsigned char sh_rank[kWarps][32];   // per warp: lane of the r-th team-sized descriptor of the ticket
     SlotRow *cache = reinterpret_cast<SlotRow *>(dyn_smem + kSmemStages);
@@ -358,11 +359,11 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // the second ticket of every warp and the descriptors of the first are requested before
     // the barrier so that their latencies hide behind it.  Tickets are index ranges only;
     // nothing is written before the batch is known to be valid.
-    unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0, cnt1 = 0;
-    if (lane == 0 && a.hand_out != kHandOutStatic) {
-        cnt1 = ticket_size(n, static_end);
-        first1 = static_end + atomicAdd(&ctl->next_desc, cnt1);
-    }
+    // (ONE atomic per CTA for its eight warps' second tickets: 2368 same-address atomics at once
+    // take microseconds to drain, and the CTA's arrival at the barrier waits for its own)
+    unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0;
+    unsigned cnt1 = a.hand_out != kHandOutStatic ? ticket_size(n, static_end) : 0u, base1 = 0;
+    if (tid == 0 && a.hand_out != kHandOutStatic) base1 = atomicAdd(&ctl->next_desc, cnt1 * kWarps);
     uint4 flo = make_uint4(0, 0, 0, 0), fhi = flo;
     const bool fhave = (unsigned)lane < cnt_static && first0 + lane < n;
     if (fhave) load_desc_raw(a.descs + first0 + lane, flo, fhi);
@@ -379,6 +380,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     unsigned long long sync = 0;
     if (a.skip_barrier) {
         // host-validated table without large descriptors: nothing to agree on, nothing to wait for
+        if (tid == 0) sh_first1 = static_end + base1;
         __syncthreads();
     } else {
         // only CTAs that validated a tile have anything to say: the others wait for the verdict
@@ -406,6 +408,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             unsigned long long v;
             while (((v = ld_acquire(&ctl->sync)) & kSyncFieldMask) < arrivals) {}
             sh_sync = v;
+            sh_first1 = static_end + base1;
         }
         __syncthreads();
         sync = sh_sync;
@@ -495,8 +498,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         // being copied, the descriptors of k+1 are being loaded, the atomic of k+2 is on its
         // way, so neither latency is exposed between two copies.
         TRACE(3);
-        first1 = __shfl_sync(0xffffffffu, first1, 0);
-        cnt1 = __shfl_sync(0xffffffffu, cnt1, 0);
+        first1 = sh_first1 + warp * cnt1;
         // Team-sized descriptors (the CTAs' votes, or the host's own count) are latency-bound, not
         // bandwidth-bound: equal counts are balanced enough, and 2368 warps drawing tickets from
         // one cursor would serialise on it (measured: 5-10 us per batch of 65,536).  They are
