@@ -137,6 +137,7 @@ struct EngineArgs {
     uint32_t flag;                   // rec_flag(sequence number of this batch)
     uint32_t gss;                    // guided self-scheduling divisor: ticket = left / (gss x warps)
     uint32_t max_group;              // units per warp ticket, at most (<= kMaxGroup)
+    uint32_t min_group;              // ... and at least
     uint32_t prefetch;               // descriptors per warp whose source is prefetched into L2 before the barrier
     uint32_t skip_barrier;           // the host validated the table and it holds no large descriptor
     uint32_t hand_out;               // kHandOutVote (device tables), or what the host's own count says
@@ -268,7 +269,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // from the end of the static tickets.
     const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
     const unsigned gdiv = a.gss * nw, gmax = a.max_group;
-    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, 1u), gmax); };
+    const unsigned gmin = a.min_group;
+    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, gmin), gmax); };
     // (a multiple of 8 when it can be: team-sized descriptors are copied 8 at a time)
     const unsigned cnt_static0 = ticket_size(n, 0), cnt_static = cnt_static0 >= 8 ? cnt_static0 & ~7u : cnt_static0;
     const unsigned static_end = nw * cnt_static;
@@ -677,6 +679,8 @@ int engine_setup(hicr_ctx *ctx)
     if (e && *e) ctx->gss = (uint32_t)std::max(1, atoi(e));
     e = getenv("HICR_MAX_GROUP");
     if (e && *e) ctx->max_group = (uint32_t)std::max(1, std::min((int)kMaxGroup, atoi(e)));
+    e = getenv("HICR_MIN_GROUP");
+    if (e && *e) ctx->min_group = (uint32_t)std::max(1, std::min((int)ctx->max_group, atoi(e)));
     e = getenv("HICR_ZERO_COPY");
     if (e && *e) ctx->zero_copy_descs = strtoull(e, nullptr, 0);
     e = getenv("HICR_PREFETCH");
@@ -750,6 +754,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     a.flag = rec_flag(ctx->batch_seq + 1);
     a.gss = ctx->gss;
     a.max_group = ctx->max_group;
+    a.min_group = ctx->min_group;
     a.prefetch = ctx->prefetch;
     a.skip_barrier = skip_barrier ? 1u : 0u;
     a.hand_out = hand_out;

@@ -533,6 +533,7 @@ struct hicr_ctx {
     uint32_t gss = 3;                        // HICR_GSS: guided self-scheduling divisor of the warp tickets
     uint32_t max_group = hicr::kMaxGroup;    // HICR_MAX_GROUP: units per warp ticket, at most
     uint64_t zero_copy_descs = hicr::kZeroCopyDescs;   // HICR_ZERO_COPY: host tables up to this long are read in place
+    uint32_t min_group = 1;                  // HICR_MIN_GROUP: units per warp ticket, at least
     uint32_t prefetch = 2;                   // HICR_PREFETCH: descriptors per warp whose source goes to L2 before the barrier
 
     bool profiling = false;
