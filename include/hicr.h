@@ -39,11 +39,15 @@ extern "C" {
 #define HICR_ERR_NO_CAPACITY      (-5)  /* slot table / work queue / allocation exhausted    */
 #define HICR_ERR_CUDA             (-6)  /* a CUDA runtime call failed; hicr_last_cuda_error  */
 #define HICR_ERR_BUSY             (-7)  /* object still referenced (e.g. slot used by a channel) */
+#define HICR_ERR_ILLEGAL_DIRECTION (-8) /* "Global-to-Global operations are not permitted"
+                                                                               */
 
 typedef struct hicr_ctx hicr_ctx_t;          /* opaque context  */
 typedef struct hicr_channel hicr_channel_t;  /* opaque SPSC channel */
 typedef struct hicr_mpsc hicr_mpsc_t;        /* opaque non-locking MPSC channel set */
-typedef uint32_t hicr_slot_t;                /* dense slot id, valid for one context */
+typedef uint32_t hicr_slot_t;                /* slot id, valid for one context: dense (0, 1, 2, ...) until
+                                                ids are recycled -- {generation:20 | table index:12},
+                                                an unregistered id is never valid again */
 
 #define HICR_MAX_SLOTS 4096u
 
@@ -85,7 +89,7 @@ const char *hicr_last_cuda_error(hicr_ctx_t *ctx);
  * allowed (then dev_ptr may be NULL).  Sent/received counters start at 0.  *out
  * receives a dense id.  Errors: HICR_ERR_UNSUPPORTED_SPACE if dev_ptr is not device
  * memory of this context's device; HICR_ERR_NO_CAPACITY beyond HICR_MAX_SLOTS live
- * and retired ids. */
+ * slots (an unregistered slot's table index is handed out again, under a new id). */
 int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_t *out);
 
 /* Forget a slot (storage untouched).  The caller must have fenced every transfer that
@@ -212,14 +216,18 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
 int hicr_mpsc_destroy(hicr_mpsc_t *m);
 int hicr_mpsc_counters(hicr_mpsc_t *m, uint32_t producer, uint64_t *head, uint64_t *tail);
 
-/* Device-resident MPSC run: one producer CTA per producer (one per SM on B200 when
- * producers = 148) pushes tokens_per_producer tokens from src_slots[p] (offset 0) into
- * its own ring in batches of at most max_batch tokens, waiting for room on the device;
- * a single consumer CTA polls the rings round-robin and pops what is available into
- * dst_slots[p] (offset 0).  Per-producer FIFO.  src_slots / dst_slots: host pointers to
- * `producers` ids.  Blocks until done; counters as for hicr_channel_stream. */
-int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_slot_t *dst_slots,
-                     uint64_t tokens_per_producer, uint64_t max_batch);
+/* Device-resident MPSC run: producer p pushes tokens_per_producer tokens from slot src_slots[p],
+ * consecutively from byte offset src_offs[p], into its own ring in batches of at most max_batch
+ * tokens, waiting for room on the device; the single logical consumer pops what is available
+ * into dst_slots[p], consecutively from dst_offs[p].  Per-producer FIFO.  head_p and tail_p
+ * continue from where the previous run left them (token i of the ring's lifetime sits at ring
+ * position i mod capacity).  src_slots / dst_slots: host pointers to
+ * `producers` ids; src_offs / dst_offs: host pointers to `producers` byte offsets, or NULL for
+ * all zero.  Requires head_p == tail_p at entry.  Blocks until done; counters as for
+ * hicr_channel_stream. */
+int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_t *src_offs,
+                     const hicr_slot_t *dst_slots, const uint64_t *dst_offs, uint64_t tokens_per_producer,
+                     uint64_t max_batch);
 
 /* Device-resident LOCKING MPSC run ("locking, where a collective exclusive
  * access guarantees a shared channel does not overflow"): `producers` producer CTAs push

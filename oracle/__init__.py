@@ -35,8 +35,12 @@ DESC_DTYPE = np.dtype(
 )
 assert DESC_DTYPE.itemsize == 32
 
+_PM_SRC = os.path.join(_HERE, "parallel_memcpy.c")
+_PM_LIB = os.path.join(_HERE, "libparallel_memcpy.so")
+
 _lock = threading.Lock()
 _lib = None
+_pm_lib = None
 
 
 def build(force: bool = False) -> str:
@@ -48,7 +52,29 @@ def build(force: bool = False) -> str:
                 ["gcc", "-O2", "-std=c99", "-Wall", "-Wextra", "-shared", "-fPIC", "-o", tmp, _SRC]
             )
             os.replace(tmp, _LIB)
+        if force or not os.path.exists(_PM_LIB) or os.path.getmtime(_PM_LIB) < os.path.getmtime(_PM_SRC):
+            tmp = _PM_LIB + ".tmp.%d" % os.getpid()
+            subprocess.check_call(
+                ["gcc", "-O2", "-std=c11", "-Wall", "-Wextra", "-shared", "-fPIC", "-pthread", "-o", tmp, _PM_SRC]
+            )
+            os.replace(tmp, _PM_LIB)
     return _LIB
+
+
+def parallel_memcpy_batch(images, descs: np.ndarray, threads: int) -> None:
+    """The stronger CPU baseline of SURVEY.md S8(d) (parallel_memcpy.c): libc memcpy per
+    descriptor over ``threads`` host threads.  Timing baseline only -- no validation, no
+    counters; ``descs`` must be a set the oracle accepts and that meets the epoch precondition."""
+    global _pm_lib
+    if _pm_lib is None:
+        build()
+        _pm_lib = ctypes.CDLL(_PM_LIB)
+        _pm_lib.parallel_memcpy_batch.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int]
+    assert descs.dtype == DESC_DTYPE and descs.flags.c_contiguous
+    bases = (ctypes.c_void_p * len(images))(*[a.ctypes.data if a.size else 0 for a in images])
+    rc = _pm_lib.parallel_memcpy_batch(bases, descs.ctypes.data, descs.size, int(threads))
+    if rc != 0:
+        raise RuntimeError("parallel_memcpy_batch: could not start its threads")
 
 
 def _load():

@@ -1,7 +1,8 @@
 """B200-native HiCR memory-slot copy engine and token channels (arxiv 2509.01425).
 
 The product is the C-ABI library declared in ``include/hicr.h`` and built from
-``csrc/*.cu`` for sm_100a; ``binding`` marshals arguments into it with ctypes.
+``csrc/*.cu`` for sm_100a; ``binding`` marshals arguments into it (ctypes, and the CPython C
+API for the calls of a step).
 Importing this package loads (building if stale) ``libhicr_b200.so`` and raises if that
 is impossible: there is no CPU fallback and nothing here imports ``oracle/``.
 """
@@ -10,6 +11,7 @@ from .binding import (  # noqa: F401
     EXPORTS,
     HICR_ERR_BUSY,
     HICR_ERR_CUDA,
+    HICR_ERR_ILLEGAL_DIRECTION,
     HICR_ERR_INVALID_ARG,
     HICR_ERR_INVALID_SLOT,
     HICR_ERR_NO_CAPACITY,

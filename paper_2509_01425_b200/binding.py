@@ -26,6 +26,7 @@ HICR_ERR_UNSUPPORTED_SPACE = -4
 HICR_ERR_NO_CAPACITY = -5
 HICR_ERR_CUDA = -6
 HICR_ERR_BUSY = -7
+HICR_ERR_ILLEGAL_DIRECTION = -8
 HICR_MAX_SLOTS = 4096
 
 # hicr_desc_t: dst_slot, src_slot, dst_off, src_off, size (PAPER.md:532 argument order)
@@ -76,7 +77,7 @@ def _load() -> ctypes.CDLL:
         "hicr_mpsc_create": (i32, [vp, u32, vp, u64, u64, P(vp)]),
         "hicr_mpsc_destroy": (i32, [vp]),
         "hicr_mpsc_counters": (i32, [vp, u32, P(u64), P(u64)]),
-        "hicr_mpsc_stream": (i32, [vp, vp, vp, u64, u64]),
+        "hicr_mpsc_stream": (i32, [vp, vp, vp, vp, vp, u64, u64]),
         "hicr_mpsc_locking_stream": (i32, [vp, u32, vp, u32, u64, u64, u64]),
         "hicr_launch_count": (i32, [vp, P(u64)]),
         "hicr_profile_enable": (i32, [vp, i32]),
@@ -90,6 +91,9 @@ def _load() -> ctypes.CDLL:
 
 lib = _load()
 LIB_PATH = _build.LIB
+# the calls of a step, through the CPython C API instead of ctypes (csrc/hicr_pyext.c); the
+# extension links against the library loaded above
+from . import _hicr_step as _step  # noqa: E402
 
 
 class HicrError(RuntimeError):
@@ -119,10 +123,9 @@ class Context:
         if rc != HICR_OK:
             raise HicrError(rc, "hicr_init")
         self._h = h
+        self._hv = h.value   # the handle as a plain int, for the C-API entry points
         self._keep = {}      # slot id -> object that owns the storage (kept alive)
         self._children = []
-        self._bad = ctypes.c_uint64(0)          # out-argument of hicr_memcpy_batch, reused across calls
-        self._bad_ref = ctypes.byref(self._bad)
 
     # ---- plumbing
     def close(self):
@@ -186,39 +189,31 @@ class Context:
         """hicr_memcpy_batch.  ``descs``: numpy array of DESC_DTYPE (host table), or a
         torch CUDA tensor / int device address of ``n`` 32-byte descriptors (device
         table; must stay alive until the fence)."""
-        if type(descs) is int:                  # device address: the hot path, nothing to marshal
-            rc = lib.hicr_memcpy_batch(self._h, descs, n, 1, self._bad_ref)
-            if rc != HICR_OK:
-                self._fail(rc, "hicr_memcpy_batch", first_bad=self._bad.value)
-            return
-        bad = ctypes.c_uint64(0)
-        if isinstance(descs, np.ndarray):
+        if type(descs) is int:                  # device address: nothing to marshal
+            ptr, cnt, dev = descs, n, 1
+        elif isinstance(descs, np.ndarray):
             if descs.dtype != DESC_DTYPE or not descs.flags.c_contiguous:
                 raise ValueError("host descriptor table must be a contiguous DESC_DTYPE array")
             cnt = descs.size if n is None else int(n)
-            rc = lib.hicr_memcpy_batch(self._h, ctypes.c_void_p(descs.ctypes.data if cnt else 0), cnt, 0,
-                                       ctypes.byref(bad))
+            ptr, dev = (descs.ctypes.data if cnt else 0), 0
         else:
-            if isinstance(descs, int):
-                ptr, cnt = descs, int(n)
-            else:
-                nbytes = descs.numel() * descs.element_size()
-                cnt = nbytes // 32 if n is None else int(n)
-                ptr = descs.data_ptr() if cnt else 0
-            rc = lib.hicr_memcpy_batch(self._h, ctypes.c_void_p(ptr), cnt, 1, ctypes.byref(bad))
-        if rc != HICR_OK:
-            self._fail(rc, "hicr_memcpy_batch", first_bad=bad.value)
+            nbytes = descs.numel() * descs.element_size()
+            cnt = nbytes // 32 if n is None else int(n)
+            ptr, dev = (descs.data_ptr() if cnt else 0), 1
+        r = _step.memcpy_batch(self._hv, ptr, cnt, dev)
+        if r:
+            self._fail(r[0], "hicr_memcpy_batch", first_bad=r[1])
 
     def fence(self):
-        rc = lib.hicr_fence(self._h)
-        if rc != HICR_OK:
+        rc = _step.fence(self._hv)
+        if rc:
             b, i = ctypes.c_uint64(), ctypes.c_uint64()
             lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
             self._fail(rc, "hicr_fence", first_bad=i.value, batch_index=b.value)
 
     def fence_async(self):
-        rc = lib.hicr_fence_async(self._h)
-        if rc != HICR_OK:
+        rc = _step.fence_async(self._hv)
+        if rc:
             self._fail(rc, "hicr_fence_async")
 
     def fence_expected(self, slot: int, sent: int, recv: int):
@@ -274,12 +269,12 @@ class Channel:
     """SPSC channel handle (hicr_channel_*)."""
 
     def __init__(self, ctx: Context, h):
-        self._ctx, self._h = ctx, h
+        self._ctx, self._h, self._hv = ctx, h, h.value
 
     def close(self):
         if self._h:
             lib.hicr_channel_destroy(self._h)
-            self._h = None
+            self._h = self._hv = None
             if self in self._ctx._children:
                 self._ctx._children.remove(self)
 
@@ -291,18 +286,16 @@ class Channel:
         return a.value, b.value
 
     def push(self, src: int, src_off: int, n_tokens: int) -> int:
-        k = ctypes.c_uint64()
-        rc = lib.hicr_channel_push(self._h, src, src_off, n_tokens, ctypes.byref(k))
-        if rc != HICR_OK:
-            self._ctx._fail(rc, "hicr_channel_push")
-        return k.value
+        k = _step.channel_push(self._hv, src, src_off, n_tokens)
+        if k < 0:
+            self._ctx._fail(k, "hicr_channel_push")
+        return k
 
     def pop(self, dst: int, dst_off: int, max_tokens: int) -> int:
-        k = ctypes.c_uint64()
-        rc = lib.hicr_channel_pop(self._h, dst, dst_off, max_tokens, ctypes.byref(k))
-        if rc != HICR_OK:
-            self._ctx._fail(rc, "hicr_channel_pop")
-        return k.value
+        k = _step.channel_pop(self._hv, dst, dst_off, max_tokens)
+        if k < 0:
+            self._ctx._fail(k, "hicr_channel_pop")
+        return k
 
     def locking_stream(self, src_slots, dst: int, dst_off: int, tokens_per_producer: int, max_batch: int):
         """hicr_mpsc_locking_stream: len(src_slots) producers share this channel's ring."""
@@ -340,11 +333,18 @@ class Mpsc:
             self._ctx._fail(rc, "hicr_mpsc_counters")
         return a.value, b.value
 
-    def stream(self, src_slots, dst_slots, tokens_per_producer: int, max_batch: int):
+    def stream(self, src_slots, dst_slots, tokens_per_producer: int, max_batch: int, src_offs=None, dst_offs=None):
         s, d = _slot_ids(src_slots), _slot_ids(dst_slots)
         if s.size != self.producers or d.size != self.producers:
             raise ValueError("need one source and one sink slot per producer")
-        rc = lib.hicr_mpsc_stream(self._h, ctypes.c_void_p(s.ctypes.data), ctypes.c_void_p(d.ctypes.data),
+        offs = []
+        for o in (src_offs, dst_offs):
+            a = None if o is None else np.ascontiguousarray(np.asarray(o, dtype=np.uint64))
+            if a is not None and a.size != self.producers:
+                raise ValueError("need one offset per producer")
+            offs.append(a)
+        so, do = (ctypes.c_void_p(a.ctypes.data) if a is not None else None for a in offs)
+        rc = lib.hicr_mpsc_stream(self._h, ctypes.c_void_p(s.ctypes.data), so, ctypes.c_void_p(d.ctypes.data), do,
                                   tokens_per_producer, max_batch)
         if rc != HICR_OK:
             self._ctx._fail(rc, "hicr_mpsc_stream")

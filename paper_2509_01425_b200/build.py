@@ -1,4 +1,5 @@
-"""Build step: compile csrc/*.cu into libhicr_b200.so for sm_100a with nvcc (in-tree).
+"""Build step: compile csrc/*.cu into libhicr_b200.so for sm_100a with nvcc (in-tree), and
+csrc/hicr_pyext.c (CPython entry points of the calls of a step) into _hicr_step.*.so with gcc.
 
 ``python -m paper_2509_01425_b200.build [--force]`` or ``build()`` from Python.  nvcc
 cross-compiles without a GPU; the .so is git-ignored but travels to the GPU box.
@@ -10,11 +11,14 @@ import os
 import shutil
 import subprocess
 import sys
+import sysconfig
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libhicr_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
+PYEXT_SRC = os.path.join(CSRC, "hicr_pyext.c")
+PYEXT = os.path.join(HERE, "_hicr_step" + (sysconfig.get_config_var("EXT_SUFFIX") or ".so"))
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -40,10 +44,24 @@ def _deps():
 
 
 def is_stale() -> bool:
-    if not os.path.exists(LIB):
+    if not os.path.exists(LIB) or not os.path.exists(PYEXT):
         return True
-    t = os.path.getmtime(LIB)
-    return any(os.path.getmtime(f) > t for f in _deps())
+    t = min(os.path.getmtime(LIB), os.path.getmtime(PYEXT))
+    return any(os.path.getmtime(f) > t for f in _deps() + [PYEXT_SRC])
+
+
+def _build_pyext() -> str:
+    """The CPython extension links against the library beside it (rpath $ORIGIN)."""
+    tmp = PYEXT + ".tmp.%d" % os.getpid()
+    cmd = ["gcc", "-O2", "-shared", "-fPIC", "-Wall", "-Wextra", "-I", sysconfig.get_paths()["include"], "-I", INCLUDE,
+           "-o", tmp, PYEXT_SRC, "-L", HERE, "-l:" + os.path.basename(LIB), "-Wl,-rpath,$ORIGIN"]
+    try:
+        subprocess.check_call(cmd)
+        os.replace(tmp, PYEXT)
+    finally:
+        if os.path.exists(tmp):
+            os.remove(tmp)
+    return PYEXT
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -58,6 +76,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     finally:
         if os.path.exists(tmp):
             os.remove(tmp)
+    _build_pyext()
     return LIB
 
 

@@ -24,20 +24,24 @@
 
 struct hicr_channel {
     hicr_ctx *ctx = nullptr;
-    hicr_slot_t ring = 0;
+    uint32_t ring = 0;             // table index of the ring slot
     uint64_t T = 0, C = 0;
     hicr::ChannelState *d_state = nullptr;
     unsigned int *d_ticket = nullptr;
     uint64_t head = 0, tail = 0;   // host mirror as of the last completed call
+    // device scratch of the device-resident runs, kept between calls (grown on demand)
+    unsigned char *d_tab = nullptr;
+    size_t tab_bytes = 0;
 };
 
 struct hicr_mpsc {
     hicr_ctx *ctx = nullptr;
     uint32_t P = 0;
     uint64_t T = 0, C = 0;
-    std::vector<hicr_slot_t> rings;
+    std::vector<uint32_t> rings;             // table indices of the ring slots
     hicr::ChannelState *d_state = nullptr;   // [P]
-    uint64_t *d_ptrs = nullptr;              // [3 * P]: ring base, source base, sink base
+    uint64_t *d_ptrs = nullptr;              // [4 * P] u64: ring base, source address, sink address, tokens before the run;
+                                             // then [3 * P] u32: table indices of ring, source, sink
     std::vector<uint64_t> head, tail;
 };
 
@@ -251,12 +255,12 @@ spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C
     }
 }
 
-// Device-resident non-locking MPSC run.  ptrs = [ring base | source base | sink base] x P.
-// slot_ids = [ring | source | sink] x P for the message counters.
+// Device-resident non-locking MPSC run.  ptrs = [ring base | source address | sink address | tokens
+// through the ring before this run] x P; slot_ids = [ring | source | sink] x P (table indices) for
+// the message counters.  head/tail keep counting from where the last run (or call) left them.
 __global__ void __launch_bounds__(kMpscThreads, 2)
 mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const uint64_t *__restrict__ ptrs,
-                   const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch,
-                   unsigned long long *sent, unsigned long long *recv, int use_tma)
+                   const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch, SlotCnt *cnt, int use_tma)
 {
     extern __shared__ __align__(128) unsigned char dyn_smem[];   // consumer, use_tma: [warp][stage][kMpscPiece]
     __shared__ uint64_t bars[(kMpscThreads / 32) * kMpscStages];
@@ -307,19 +311,21 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
         for (uint32_t p = warp; p < P; p += nwarps) {
             ChannelState *s = st + p;
             unsigned long long tail = 0, head = 0;
+            const unsigned long long end = ptrs[3 * P + p] + tokens;   // tail when this run is through
             if (lane == 0) {
                 tail = __ldcg(&s->tail);   // only this warp ever writes it (read at L2, where the release store went)
-                head = tail < tokens ? ld_acquire(&s->head) : tail;
+                head = tail < end ? ld_acquire(&s->head) : tail;
             }
             tail = __shfl_sync(0xffffffffu, tail, 0);
             head = __shfl_sync(0xffffffffu, head, 0);
-            if (tail >= tokens) continue;
+            if (tail >= end) continue;
             all_done = false;
             const uint64_t k = head - tail;
             if (k == 0) continue;
             progressed = true;
             unsigned char *ring = reinterpret_cast<unsigned char *>(ptrs[p]);
-            unsigned char *dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]);
+            // sink address of the token at ring count `tail`
+            unsigned char *dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]) - (end - tokens) * T;
             if (use_tma) {
                 // bulk copies ring -> shared -> sink, up to kMpscStages loads in flight; when the call
                 // returns the ring bytes have been read, so the tail can move while the stores drain
@@ -335,11 +341,11 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
             __syncwarp();
             if (lane == 0) {
                 st_release(&s->tail, tail + k);
-                if (tail + k == tokens) {   // this ring is through: one message per token (reading 15)
-                    atomicAdd(&sent[slot_ids[P + p]], (unsigned long long)tokens);
-                    atomicAdd(&recv[slot_ids[p]], (unsigned long long)tokens);
-                    atomicAdd(&sent[slot_ids[p]], (unsigned long long)tokens);
-                    atomicAdd(&recv[slot_ids[2 * P + p]], (unsigned long long)tokens);
+                if (tail + k == end) {   // this ring is through: one message per token (reading 15)
+                    atomicAdd(&cnt[slot_ids[P + p]].sent, (unsigned long long)tokens);
+                    atomicAdd(&cnt[slot_ids[p]].recv, (unsigned long long)tokens);
+                    atomicAdd(&cnt[slot_ids[p]].sent, (unsigned long long)tokens);
+                    atomicAdd(&cnt[slot_ids[2 * P + p]].recv, (unsigned long long)tokens);
                 }
             }
         }
@@ -360,8 +366,8 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
 __global__ void __launch_bounds__(kMpscThreads, 2)
 mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, unsigned char *ring, uint64_t T,
                     uint64_t C, const uint64_t *__restrict__ srcs, const uint32_t *__restrict__ slot_ids,
-                    unsigned char *dst, uint64_t tokens, uint64_t max_batch, unsigned long long *sent,
-                    unsigned long long *recv, uint32_t ring_slot, uint32_t dst_slot, CallResult *res)
+                    unsigned char *dst, uint64_t tokens, uint64_t max_batch, SlotCnt *cnt, uint32_t ring_slot,
+                    uint32_t dst_slot, CallResult *res)
 {
     __shared__ unsigned long long sh_start, sh_k;
     const uint64_t ring_bytes = C * T;
@@ -400,7 +406,7 @@ mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, u
             }
             pushed += k;
         }
-        if (tid == 0) atomicAdd(&sent[slot_ids[p]], (unsigned long long)tokens);
+        if (tid == 0) atomicAdd(&cnt[slot_ids[p]].sent, (unsigned long long)tokens);
         return;
     }
     // ---- the single consumer
@@ -424,9 +430,9 @@ mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, u
         popped += k;
     }
     if (tid == 0) {
-        atomicAdd(&recv[ring_slot], (unsigned long long)total);
-        atomicAdd(&sent[ring_slot], (unsigned long long)total);
-        atomicAdd(&recv[dst_slot], (unsigned long long)total);
+        atomicAdd(&cnt[ring_slot].recv, (unsigned long long)total);
+        atomicAdd(&cnt[ring_slot].sent, (unsigned long long)total);
+        atomicAdd(&cnt[dst_slot].recv, (unsigned long long)total);
         res->k = total;
         res->head = tail0 + total;
         res->tail = tail;
@@ -447,9 +453,25 @@ static CallResult read_result(hicr_ctx *ctx)
     return r;
 }
 
-static int slot_ok(hicr_ctx *ctx, hicr_slot_t s)
+// Device scratch of a channel's device-resident runs: at least `bytes`, contents undefined.
+static int channel_scratch(hicr_channel *ch, size_t bytes)
 {
-    return s < ctx->slots.size() && ctx->slots[s].size != kInvalidSize;
+    if (bytes <= ch->tab_bytes) return HICR_OK;
+    hicr_ctx *ctx = ch->ctx;
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
+    if (ch->d_tab) HICR_CUDA(ctx, cudaFree(ch->d_tab));
+    ch->d_tab = nullptr;
+    ch->tab_bytes = 0;
+    const size_t cap = std::max<size_t>(bytes, 1 << 16);
+    HICR_CUDA(ctx, cudaMalloc(&ch->d_tab, cap));
+    ch->tab_bytes = cap;
+    return HICR_OK;
+}
+
+// Overflow-safe "count tokens of T bytes fit into [off, size)".
+static bool tokens_fit(uint64_t count, uint64_t T, uint64_t off, uint64_t size)
+{
+    return off <= size && (count == 0 || (count <= ~0ull / T && count * T <= size - off));
 }
 
 }  // namespace hicr
@@ -464,13 +486,13 @@ int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes,
     if (!ctx || !out) return HICR_ERR_INVALID_ARG;
     *out = nullptr;
     if (token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;   // capacity >= 1
-    if (!slot_ok(ctx, ring)) return HICR_ERR_INVALID_SLOT;
-    if (capacity > ~0ull / token_bytes || capacity * token_bytes > ctx->slots[ring].size)
-        return HICR_ERR_OUT_OF_BOUNDS;
+    const int64_t ri = slot_find(ctx, ring);
+    if (ri < 0) return HICR_ERR_INVALID_SLOT;
+    if (!tokens_fit(capacity, token_bytes, 0, row_size(ctx->rows[ri]))) return HICR_ERR_OUT_OF_BOUNDS;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     hicr_channel *ch = new hicr_channel();
     ch->ctx = ctx;
-    ch->ring = ring;
+    ch->ring = (uint32_t)ri;
     ch->T = token_bytes;
     ch->C = capacity;
     cudaError_t e = cudaMalloc(&ch->d_state, sizeof(ChannelState) + 128);
@@ -481,7 +503,7 @@ int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes,
         return cuda_fail(ctx, e, "hicr_channel_create");
     }
     ch->d_ticket = reinterpret_cast<unsigned int *>(ch->d_state + 1);
-    ctx->ring_refs[ring]++;
+    ctx->ring_refs[ri]++;
     *out = ch;
     return HICR_OK;
 }
@@ -491,6 +513,7 @@ int hicr_channel_destroy(hicr_channel_t *ch)
     if (!ch) return HICR_ERR_INVALID_ARG;
     (void)cudaStreamSynchronize(ch->ctx->stream);
     cudaFree(ch->d_state);
+    cudaFree(ch->d_tab);
     ch->ctx->ring_refs[ch->ring]--;
     delete ch;
     return HICR_OK;
@@ -510,30 +533,30 @@ static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uin
     if (!ch || !n_out) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = ch->ctx;
     *n_out = 0;
-    if (!slot_ok(ctx, lin_slot)) return HICR_ERR_INVALID_SLOT;
-    const SlotRow &ls = ctx->slots[lin_slot];
-    if (off > ls.size) return HICR_ERR_OUT_OF_BOUNDS;
-    if (push) {
-        if (n > ~0ull / ch->T || n * ch->T > ls.size - off) return HICR_ERR_OUT_OF_BOUNDS;
-    }
+    const int64_t li = slot_find(ctx, lin_slot);
+    if (li < 0) return HICR_ERR_INVALID_SLOT;
+    const SlotRow &ls = ctx->rows[li];
+    const uint64_t lsize = row_size(ls);
+    if (off > lsize) return HICR_ERR_OUT_OF_BOUNDS;
+    if (push && !tokens_fit(n, ch->T, off, lsize)) return HICR_ERR_OUT_OF_BOUNDS;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     const uint64_t max_tokens = std::min<uint64_t>(n, ch->C);
     const uint64_t max_bytes = max_tokens * ch->T;
     unsigned grid = (unsigned)std::min<uint64_t>(std::max<uint64_t>(1, (max_bytes + kPieceBytes - 1) / kPieceBytes),
                                                  (uint64_t)ctx->num_sms * 4);
-    unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+    unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->rows[ch->ring].base);
     unsigned char *lin = reinterpret_cast<unsigned char *>(ls.base + off);
     CallResult *res = ctx->d_call;
     const unsigned long long seq = ++ctx->call_seq;
+    SlotCnt *cl = ctx->d_cnt + li, *cr = ctx->d_cnt + ch->ring;
     if (push)
         channel_call_kernel<true><<<grid, kCallThreads, 0, ctx->stream>>>(
-            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_sent + lin_slot,
-            ctx->d_recv + ch->ring, res, seq);
+            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->sent, &cr->recv, res, seq);
     else
         channel_call_kernel<false><<<grid, kCallThreads, 0, ctx->stream>>>(
-            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, ls.size - off, n, ctx->d_recv + lin_slot,
-            ctx->d_sent + ch->ring, res, seq);
+            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->recv, &cr->sent, res, seq);
     ctx->launches++;
+    ctx->push_stale = true;   // the device counters moved after the last batch's pushed snapshot
     HICR_CUDA(ctx, cudaGetLastError());
     // "Complete on return": the last CTA writes the result as flagged words, which the host polls
     // (4.5 us less per call than cudaStreamSynchronize); every so often the stream is asked,
@@ -569,11 +592,11 @@ static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uin
     if (r.status != HICR_OK) return (int)r.status;
     *n_out = r.k;
     if (push) {
-        ctx->sent[lin_slot] += r.k;
-        ctx->recv[ch->ring] += r.k;
+        ctx->cnt[li].sent += r.k;
+        ctx->cnt[ch->ring].recv += r.k;
     } else {
-        ctx->sent[ch->ring] += r.k;
-        ctx->recv[lin_slot] += r.k;
+        ctx->cnt[ch->ring].sent += r.k;
+        ctx->cnt[li].recv += r.k;
     }
     return HICR_OK;
 }
@@ -593,7 +616,8 @@ int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, h
 {
     if (!ch || (!batch_tokens && n_batches)) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = ch->ctx;
-    if (!slot_ok(ctx, src) || !slot_ok(ctx, dst)) return HICR_ERR_INVALID_SLOT;
+    const int64_t si = slot_find(ctx, src), di = slot_find(ctx, dst);
+    if (si < 0 || di < 0) return HICR_ERR_INVALID_SLOT;
     if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;
     uint64_t total = 0;
     for (uint64_t i = 0; i < n_batches; i++) {
@@ -601,40 +625,39 @@ int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, h
         total += batch_tokens[i];
         if (total > (1ull << 48)) return HICR_ERR_OUT_OF_BOUNDS;
     }
-    const SlotRow &ss = ctx->slots[src], &ds = ctx->slots[dst];
-    if (total > ~0ull / ch->T) return HICR_ERR_OUT_OF_BOUNDS;
-    if (src_off > ss.size || total * ch->T > ss.size - src_off) return HICR_ERR_OUT_OF_BOUNDS;
-    if (dst_off > ds.size || total * ch->T > ds.size - dst_off) return HICR_ERR_OUT_OF_BOUNDS;
+    const SlotRow &ss = ctx->rows[si], &ds = ctx->rows[di];
+    if (!tokens_fit(total, ch->T, src_off, row_size(ss)) || !tokens_fit(total, ch->T, dst_off, row_size(ds)))
+        return HICR_ERR_OUT_OF_BOUNDS;
     if (total == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
-    uint64_t *d_batches = nullptr;
-    HICR_CUDA(ctx, cudaMalloc(&d_batches, n_batches * 8));
-    cudaError_t e = cudaMemcpyAsync(d_batches, batch_tokens, n_batches * 8, cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) {
+    int rc = channel_scratch(ch, n_batches * 8);
+    if (rc != HICR_OK) return rc;
+    uint64_t *d_batches = reinterpret_cast<uint64_t *>(ch->d_tab);
+    HICR_CUDA(ctx, cudaMemcpyAsync(d_batches, batch_tokens, n_batches * 8, cudaMemcpyHostToDevice, ctx->stream));
+    {
         ChannelState *st = ch->d_state;
-        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->rows[ch->ring].base);
         unsigned char *sp = reinterpret_cast<unsigned char *>(ss.base + src_off);
         unsigned char *dp = reinterpret_cast<unsigned char *>(ds.base + dst_off);
         uint64_t T = ch->T, C = ch->C;
         const uint64_t *bp = d_batches;
-        unsigned long long *c0 = ctx->d_sent + src, *c1 = ctx->d_recv + ch->ring, *c2 = ctx->d_sent + ch->ring,
-                           *c3 = ctx->d_recv + dst;
+        unsigned long long *c0 = &ctx->d_cnt[si].sent, *c1 = &ctx->d_cnt[ch->ring].recv, *c2 = &ctx->d_cnt[ch->ring].sent,
+                           *c3 = &ctx->d_cnt[di].recv;
         CallResult *res = ctx->d_call;
         void *args[] = {&st, &ring, &T, &C, &sp, &dp, &bp, &n_batches, &total, &c0, &c1, &c2, &c3, &res};
-        e = cudaLaunchCooperativeKernel((const void *)spsc_stream_kernel, dim3(2), dim3(kStreamThreads), args, 0,
-                                        ctx->stream);
+        HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)spsc_stream_kernel, dim3(2), dim3(kStreamThreads), args, 0,
+                                                   ctx->stream));
         ctx->launches++;
+        ctx->push_stale = true;
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    cudaFree(d_batches);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "hicr_channel_stream");
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));   // also: batch_tokens has been consumed
     const CallResult r = read_result(ctx);
     ch->head = r.head;
     ch->tail = r.tail;
-    ctx->sent[src] += total;
-    ctx->recv[ch->ring] += total;
-    ctx->sent[ch->ring] += total;
-    ctx->recv[dst] += total;
+    ctx->cnt[si].sent += total;
+    ctx->cnt[ch->ring].recv += total;
+    ctx->cnt[ch->ring].sent += total;
+    ctx->cnt[di].recv += total;
     return HICR_OK;
 }
 
@@ -644,10 +667,12 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
     if (!ctx || !out || !rings) return HICR_ERR_INVALID_ARG;
     *out = nullptr;
     if (producers == 0 || token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;
-    if (capacity > ~0ull / token_bytes) return HICR_ERR_OUT_OF_BOUNDS;
+    std::vector<uint32_t> idx(producers);
     for (uint32_t p = 0; p < producers; p++) {
-        if (!slot_ok(ctx, rings[p])) return HICR_ERR_INVALID_SLOT;
-        if (capacity * token_bytes > ctx->slots[rings[p]].size) return HICR_ERR_OUT_OF_BOUNDS;
+        const int64_t ri = slot_find(ctx, rings[p]);
+        if (ri < 0) return HICR_ERR_INVALID_SLOT;
+        if (!tokens_fit(capacity, token_bytes, 0, row_size(ctx->rows[ri]))) return HICR_ERR_OUT_OF_BOUNDS;
+        idx[p] = (uint32_t)ri;
     }
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     hicr_mpsc *m = new hicr_mpsc();
@@ -655,19 +680,19 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
     m->P = producers;
     m->T = token_bytes;
     m->C = capacity;
-    m->rings.assign(rings, rings + producers);
+    m->rings = idx;
     m->head.assign(producers, 0);
     m->tail.assign(producers, 0);
     cudaError_t e = cudaMalloc(&m->d_state, sizeof(ChannelState) * producers);
     if (e == cudaSuccess) e = cudaMemsetAsync(m->d_state, 0, sizeof(ChannelState) * producers, ctx->stream);
-    if (e == cudaSuccess) e = cudaMalloc(&m->d_ptrs, (size_t)producers * (3 * 8 + 3 * 4));
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_ptrs, (size_t)producers * (4 * 8 + 3 * 4));
     if (e != cudaSuccess) {
         cudaFree(m->d_state);
         cudaFree(m->d_ptrs);
         delete m;
         return cuda_fail(ctx, e, "hicr_mpsc_create");
     }
-    for (uint32_t p = 0; p < producers; p++) ctx->ring_refs[rings[p]]++;
+    for (uint32_t p = 0; p < producers; p++) ctx->ring_refs[idx[p]]++;
     *out = m;
     return HICR_OK;
 }
@@ -691,27 +716,37 @@ int hicr_mpsc_counters(hicr_mpsc_t *m, uint32_t producer, uint64_t *head, uint64
     return HICR_OK;
 }
 
-int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_slot_t *dst_slots,
-                     uint64_t tokens_per_producer, uint64_t max_batch)
+int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_t *src_offs, const hicr_slot_t *dst_slots,
+                     const uint64_t *dst_offs, uint64_t tokens_per_producer, uint64_t max_batch)
 {
     if (!m || !src_slots || !dst_slots || max_batch == 0) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = m->ctx;
     const uint32_t P = m->P;
     const uint64_t N = tokens_per_producer;
     if (N > (1ull << 48) / m->T) return HICR_ERR_OUT_OF_BOUNDS;
+    std::vector<uint64_t> ptrs(4 * (size_t)P);
+    std::vector<uint32_t> ids(3 * (size_t)P);
+    // every ring, sink and token size a multiple of 16 bytes: the consumer moves tokens with bulk copies
+    int use_tma = m->T % 16 == 0;
     for (uint32_t p = 0; p < P; p++) {
-        if (!slot_ok(ctx, src_slots[p]) || !slot_ok(ctx, dst_slots[p])) return HICR_ERR_INVALID_SLOT;
-        if (N * m->T > ctx->slots[src_slots[p]].size || N * m->T > ctx->slots[dst_slots[p]].size)
+        const int64_t si = slot_find(ctx, src_slots[p]), di = slot_find(ctx, dst_slots[p]);
+        if (si < 0 || di < 0) return HICR_ERR_INVALID_SLOT;
+        const uint64_t so = src_offs ? src_offs[p] : 0, dof = dst_offs ? dst_offs[p] : 0;
+        if (!tokens_fit(N, m->T, so, row_size(ctx->rows[si])) || !tokens_fit(N, m->T, dof, row_size(ctx->rows[di])))
             return HICR_ERR_OUT_OF_BOUNDS;
         if (m->head[p] != m->tail[p]) return HICR_ERR_INVALID_ARG;
+        ptrs[p] = ctx->rows[m->rings[p]].base;
+        ptrs[P + p] = ctx->rows[si].base + so;
+        ptrs[2 * P + p] = ctx->rows[di].base + dof;
+        ptrs[3 * P + p] = m->tail[p];
+        ids[p] = m->rings[p];
+        ids[P + p] = (uint32_t)si;
+        ids[2 * P + p] = (uint32_t)di;
+        if ((ptrs[p] | ptrs[2 * P + p]) % 16) use_tma = 0;
     }
     if (N == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     // co-residency of all P + 1 CTAs is what makes the spin-waits safe
-    // every ring, sink and token size a multiple of 16 bytes: the consumer moves tokens with bulk copies
-    int use_tma = m->T % 16 == 0;
-    for (uint32_t p = 0; p < P && use_tma; p++)
-        use_tma = (ctx->slots[m->rings[p]].base | ctx->slots[dst_slots[p]].base) % 16 == 0;
     size_t smem = use_tma ? (size_t)(kMpscThreads / 32) * kMpscStages * kMpscPiece : 0;
     int per_sm = 0;
     if (use_tma) {
@@ -726,41 +761,29 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const hicr_sl
         HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, 0));
         if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
     }
-
-    std::vector<uint64_t> ptrs(3 * (size_t)P);
-    std::vector<uint32_t> ids(3 * (size_t)P);
-    for (uint32_t p = 0; p < P; p++) {
-        ptrs[p] = ctx->slots[m->rings[p]].base;
-        ptrs[P + p] = ctx->slots[src_slots[p]].base;
-        ptrs[2 * P + p] = ctx->slots[dst_slots[p]].base;
-        ids[p] = m->rings[p];
-        ids[P + p] = src_slots[p];
-        ids[2 * P + p] = dst_slots[p];
-    }
-    uint32_t *d_ids = reinterpret_cast<uint32_t *>(m->d_ptrs + 3 * (size_t)P);
+    uint32_t *d_ids = reinterpret_cast<uint32_t *>(m->d_ptrs + 4 * (size_t)P);
+    // (pageable sources: the runtime stages them before returning)
     HICR_CUDA(ctx, cudaMemcpyAsync(m->d_ptrs, ptrs.data(), ptrs.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
     HICR_CUDA(ctx, cudaMemcpyAsync(d_ids, ids.data(), ids.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
-    // heads/tails restart from the mirror values (they are equal per ring); the kernel
-    // works with absolute token indices, so reset the device counters to 0-based per run
-    HICR_CUDA(ctx, cudaMemsetAsync(m->d_state, 0, sizeof(ChannelState) * P, ctx->stream));
     ChannelState *st = m->d_state;
     uint32_t Pv = P;
     uint64_t T = m->T, C = m->C, tok = N, mb = max_batch;
     const uint64_t *pp = m->d_ptrs;
     const uint32_t *ip = d_ids;
-    unsigned long long *sent = ctx->d_sent, *recv = ctx->d_recv;
-    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &sent, &recv, &use_tma};
+    SlotCnt *cnt = ctx->d_cnt;
+    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &cnt, &use_tma};
     HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_stream_kernel, dim3(P + 1), dim3(kMpscThreads),
                                                args, smem, ctx->stream));
     ctx->launches++;
+    ctx->push_stale = true;
     HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (uint32_t p = 0; p < P; p++) {
         m->head[p] += N;
         m->tail[p] += N;
-        ctx->sent[src_slots[p]] += N;
-        ctx->recv[m->rings[p]] += N;
-        ctx->sent[m->rings[p]] += N;
-        ctx->recv[dst_slots[p]] += N;
+        ctx->cnt[ids[P + p]].sent += N;
+        ctx->cnt[m->rings[p]].recv += N;
+        ctx->cnt[m->rings[p]].sent += N;
+        ctx->cnt[ids[2 * P + p]].recv += N;
     }
     return HICR_OK;
 }
@@ -773,14 +796,20 @@ int hicr_mpsc_locking_stream(hicr_channel_t *ch, uint32_t producers, const hicr_
     const uint32_t P = producers;
     const uint64_t N = tokens_per_producer;
     if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;   // requires an empty ring at entry
-    if (!slot_ok(ctx, dst)) return HICR_ERR_INVALID_SLOT;
+    const int64_t di = slot_find(ctx, dst);
+    if (di < 0) return HICR_ERR_INVALID_SLOT;
     if (N > (1ull << 48) / ch->T / P) return HICR_ERR_OUT_OF_BOUNDS;
+    std::vector<uint64_t> ptrs(P);
+    std::vector<uint32_t> ids(P);
     for (uint32_t p = 0; p < P; p++) {
-        if (!slot_ok(ctx, src_slots[p])) return HICR_ERR_INVALID_SLOT;
-        if (N * ch->T > ctx->slots[src_slots[p]].size) return HICR_ERR_OUT_OF_BOUNDS;
+        const int64_t si = slot_find(ctx, src_slots[p]);
+        if (si < 0) return HICR_ERR_INVALID_SLOT;
+        if (!tokens_fit(N, ch->T, 0, row_size(ctx->rows[si]))) return HICR_ERR_OUT_OF_BOUNDS;
+        ptrs[p] = ctx->rows[si].base;
+        ids[p] = (uint32_t)si;
     }
-    const SlotRow &ds = ctx->slots[dst];
-    if (dst_off > ds.size || (uint64_t)P * N * ch->T > ds.size - dst_off) return HICR_ERR_OUT_OF_BOUNDS;
+    const SlotRow &ds = ctx->rows[di];
+    if (!tokens_fit((uint64_t)P * N, ch->T, dst_off, row_size(ds))) return HICR_ERR_OUT_OF_BOUNDS;
     if (N == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     // co-residency of all P + 1 CTAs is what makes the spin-waits (reservation, in-order commit) safe
@@ -788,48 +817,42 @@ int hicr_mpsc_locking_stream(hicr_channel_t *ch, uint32_t producers, const hicr_
     HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_locking_kernel, kMpscThreads, 0));
     if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
 
-    std::vector<uint64_t> ptrs(P);
-    std::vector<uint32_t> ids(P);
-    for (uint32_t p = 0; p < P; p++) {
-        ptrs[p] = ctx->slots[src_slots[p]].base;
-        ids[p] = src_slots[p];
-    }
-    unsigned char *d_tab = nullptr;   // [P] u64 source bases, [P] u32 slot ids, one u64 reservation counter
-    const size_t tab_bytes = (size_t)P * 12 + 16;
-    HICR_CUDA(ctx, cudaMalloc(&d_tab, tab_bytes));
+    // scratch: [P] u64 source bases, one u64 reservation counter, [P] u32 table indices
+    int rc = channel_scratch(ch, (size_t)P * 12 + 16);
+    if (rc != HICR_OK) return rc;
+    unsigned char *d_tab = ch->d_tab;
     uint64_t *d_ptrs = reinterpret_cast<uint64_t *>(d_tab);
     unsigned long long *d_reserve = reinterpret_cast<unsigned long long *>(d_tab + (size_t)P * 8);
     uint32_t *d_ids = reinterpret_cast<uint32_t *>(d_tab + (size_t)P * 8 + 8);
     const unsigned long long head0 = ch->head;
-    cudaError_t e = cudaMemcpyAsync(d_ptrs, ptrs.data(), (size_t)P * 8, cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_reserve, &head0, 8, cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(d_ids, ids.data(), (size_t)P * 4, cudaMemcpyHostToDevice, ctx->stream);
-    if (e == cudaSuccess) {
+    HICR_CUDA(ctx, cudaMemcpyAsync(d_ptrs, ptrs.data(), (size_t)P * 8, cudaMemcpyHostToDevice, ctx->stream));
+    HICR_CUDA(ctx, cudaMemcpyAsync(d_reserve, &head0, 8, cudaMemcpyHostToDevice, ctx->stream));
+    HICR_CUDA(ctx, cudaMemcpyAsync(d_ids, ids.data(), (size_t)P * 4, cudaMemcpyHostToDevice, ctx->stream));
+    {
         ChannelState *st = ch->d_state;
-        uint32_t Pv = P, ring_slot = ch->ring, dst_slot = dst;
-        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->slots[ch->ring].base);
+        uint32_t Pv = P, ring_slot = ch->ring, dst_slot = (uint32_t)di;
+        unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->rows[ch->ring].base);
         unsigned char *dp = reinterpret_cast<unsigned char *>(ds.base + dst_off);
         uint64_t T = ch->T, C = ch->C, tok = N, mb = max_batch;
         const uint64_t *pp = d_ptrs;
         const uint32_t *ip = d_ids;
-        unsigned long long *sent = ctx->d_sent, *recv = ctx->d_recv;
+        SlotCnt *cnt = ctx->d_cnt;
         CallResult *res = ctx->d_call;
-        void *args[] = {&st, &d_reserve, &Pv, &ring, &T, &C, &pp, &ip, &dp, &tok, &mb, &sent, &recv, &ring_slot, &dst_slot, &res};
-        e = cudaLaunchCooperativeKernel((const void *)mpsc_locking_kernel, dim3(P + 1), dim3(kMpscThreads), args, 0,
-                                        ctx->stream);
+        void *args[] = {&st, &d_reserve, &Pv, &ring, &T, &C, &pp, &ip, &dp, &tok, &mb, &cnt, &ring_slot, &dst_slot, &res};
+        HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_locking_kernel, dim3(P + 1), dim3(kMpscThreads), args, 0,
+                                                   ctx->stream));
         ctx->launches++;
+        ctx->push_stale = true;
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
-    cudaFree(d_tab);
-    if (e != cudaSuccess) return cuda_fail(ctx, e, "hicr_mpsc_locking_stream");
+    HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     const CallResult r = read_result(ctx);
     ch->head = r.head;
     ch->tail = r.tail;
     const uint64_t total = (uint64_t)P * N;
-    for (uint32_t p = 0; p < P; p++) ctx->sent[src_slots[p]] += N;
-    ctx->recv[ch->ring] += total;
-    ctx->sent[ch->ring] += total;
-    ctx->recv[dst] += total;
+    for (uint32_t p = 0; p < P; p++) ctx->cnt[ids[p]].sent += N;
+    ctx->cnt[ch->ring].recv += total;
+    ctx->cnt[ch->ring].sent += total;
+    ctx->cnt[di].recv += total;
     return HICR_OK;
 }
 

@@ -22,28 +22,26 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what)
     return HICR_ERR_CUDA;
 }
 
-static int bad_to_status(unsigned id)
+int bad_to_status(unsigned id)
 {
     switch (id) {
     case kBadInvalidSlot: return HICR_ERR_INVALID_SLOT;
     case kBadOutOfBounds: return HICR_ERR_OUT_OF_BOUNDS;
     case kBadNoCapacity: return HICR_ERR_NO_CAPACITY;
+    case kBadDirection: return HICR_ERR_ILLEGAL_DIRECTION;
     default: return HICR_ERR_INVALID_ARG;
     }
 }
 
-// Read back the slot counters (device -> pinned -> host mirror) and wait for the stream.
+// Read back the slot counters (device -> pinned -> host mirror) and wait for the stream: the
+// fence's slow path, for everything the pushed snapshot of the last batch does not cover.
 int refresh_counters(hicr_ctx *ctx)
 {
-    const size_t n = ctx->slots.size();
+    const size_t n = ctx->rows.size();
     if (n == 0) return HICR_OK;
-    unsigned char *p = ctx->h_fence;
-    HICR_CUDA(ctx, cudaMemcpyAsync(p, ctx->d_sent, n * 8, cudaMemcpyDeviceToHost, ctx->stream));
-    HICR_CUDA(ctx, cudaMemcpyAsync(p + 8 * (size_t)HICR_MAX_SLOTS, ctx->d_recv, n * 8, cudaMemcpyDeviceToHost,
-                                   ctx->stream));
+    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->h_fence, ctx->d_cnt, n * sizeof(SlotCnt), cudaMemcpyDeviceToHost, ctx->stream));
     HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
-    memcpy(ctx->sent.data(), p, n * 8);
-    memcpy(ctx->recv.data(), p + 8 * (size_t)HICR_MAX_SLOTS, n * 8);
+    memcpy(ctx->cnt.data(), ctx->h_fence, n * sizeof(SlotCnt));
     return HICR_OK;
 }
 
@@ -88,7 +86,7 @@ static inline uint64_t join64(uint32_t lo, uint32_t hi) { return (uint64_t)lo | 
 int drain_epoch(hicr_ctx *ctx, bool final_fence)
 {
     const uint32_t nb = ctx->batches_in_epoch;
-    const size_t n = ctx->slots.size();
+    const size_t n = ctx->rows.size();
     uint32_t words[kRwUsed];
     for (uint32_t k = 0; k < nb; k++) {
         const uint32_t b = k == 0 ? nb - 1 : k - 1;   // last batch first, then 0 .. nb-2
@@ -114,23 +112,61 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence)
     ctx->epoch_batch_base += nb;
     ctx->batches_in_epoch = 0;
     if (n && final_fence) {
-        if (nb && n <= kPushSlots) {
-            // the last batch pushed the cumulative counters next to the records
+        // The last launched batch pushed the cumulative counters of the first last_n_push table
+        // rows next to the records.  That snapshot serves the fence unless something counted, or
+        // changed the table, after that launch (a channel kernel, a registration): then the
+        // whole table is read back in stream order.
+        if (ctx->batch_seq && !ctx->push_stale && n <= ctx->last_n_push) {
             int rc = wait_words(ctx, ctx->h_rec[kRecRing].w, n * kPushWordsPerSlot, rec_flag(ctx->batch_seq),
                                 ctx->push_words.data());
             if (rc != HICR_OK) return rc;
             for (size_t s = 0; s < n; s++) {
                 const uint32_t *w = ctx->push_words.data() + s * kPushWordsPerSlot;
-                ctx->sent[s] = join64(w[0], w[1]);
-                ctx->recv[s] = join64(w[2], w[3]);
+                ctx->cnt[s].sent = join64(w[0], w[1]);
+                ctx->cnt[s].recv = join64(w[2], w[3]);
             }
         } else {
             int rc = refresh_counters(ctx);
             if (rc != HICR_OK) return rc;
         }
     }
+    // every batch of the epoch launched so far has completed, so has the staging it read
     for (auto &b : ctx->used_stage) ctx->free_stage.push_back(b);
     ctx->used_stage.clear();
+    return HICR_OK;
+}
+
+// (a1) Put one row into the slot table: the lowest free index, under its next generation, with
+// zeroed counters; stream-ordered after everything already enqueued.  flags = kRowGlobal / kRowRemote.
+int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hicr_slot_t *out)
+{
+    uint32_t i;
+    if (!ctx->free_idx.empty()) i = ctx->free_idx.back();
+    else if (ctx->rows.size() < HICR_MAX_SLOTS) i = (uint32_t)ctx->rows.size();
+    else return HICR_ERR_NO_CAPACITY;
+    const bool reuse = i < ctx->rows.size();
+    const uint32_t g = reuse ? ctx->gen[i] + 1 : 0;
+    const SlotRow row{base, row_meta(size, g, flags)};
+    // the row lives in pageable host memory, so the runtime stages it before returning
+    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + i, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
+    if (reuse) {
+        HICR_CUDA(ctx, cudaMemsetAsync(ctx->d_cnt + i, 0, sizeof(SlotCnt), ctx->stream));
+        ctx->free_idx.pop_back();
+        ctx->rows[i] = row;
+        ctx->gen[i] = g;
+        ctx->cnt[i] = SlotCnt{0, 0};
+        ctx->ring_refs[i] = 0;
+        ctx->born[i] = ctx->batch_seq;
+    } else {
+        ctx->rows.push_back(row);
+        ctx->gen.push_back(g);
+        ctx->cnt.push_back(SlotCnt{0, 0});
+        ctx->ring_refs.push_back(0);
+        ctx->born.push_back(ctx->batch_seq);
+    }
+    ctx->registered_bytes += size;
+    ctx->push_stale = true;
+    *out = (hicr_slot_t)((g << kSlotIndexBits) | i);
     return HICR_OK;
 }
 
@@ -151,6 +187,7 @@ const char *hicr_strerror(int status)
     case HICR_ERR_NO_CAPACITY: return "capacity exhausted";
     case HICR_ERR_CUDA: return "CUDA runtime error";
     case HICR_ERR_BUSY: return "object in use";
+    case HICR_ERR_ILLEGAL_DIRECTION: return "global-to-global transfers are not permitted";
     default: return "unknown status";
     }
 }
@@ -184,11 +221,9 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
     INIT_CUDA(cudaSetDevice(device));
     INIT_CUDA(cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, device));
     INIT_CUDA(cudaMalloc(&ctx->d_slots, sizeof(SlotRow) * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMemset(ctx->d_slots, 0xff, sizeof(SlotRow) * HICR_MAX_SLOTS));  // size = kInvalidSize
-    INIT_CUDA(cudaMalloc(&ctx->d_sent, 8 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMalloc(&ctx->d_recv, 8 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMemset(ctx->d_sent, 0, 8 * HICR_MAX_SLOTS));
-    INIT_CUDA(cudaMemset(ctx->d_recv, 0, 8 * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_slots, 0xff, sizeof(SlotRow) * HICR_MAX_SLOTS));  // meta = kInvalidMeta
+    INIT_CUDA(cudaMalloc(&ctx->d_cnt, sizeof(SlotCnt) * HICR_MAX_SLOTS));
+    INIT_CUDA(cudaMemset(ctx->d_cnt, 0, sizeof(SlotCnt) * HICR_MAX_SLOTS));
     INIT_CUDA(cudaMalloc(&ctx->d_ctl, sizeof(Ctl)));
     INIT_CUDA(cudaMemset(ctx->d_ctl, 0, sizeof(Ctl)));
     {
@@ -198,8 +233,7 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
         memset(ctx->h_rec, 0, rec_bytes);
         INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_rec, ctx->h_rec, 0));
     }
-    ctx->h_fence_bytes = 2 * 8 * (size_t)HICR_MAX_SLOTS;
-    INIT_CUDA(cudaHostAlloc(&ctx->h_fence, ctx->h_fence_bytes, cudaHostAllocDefault));
+    INIT_CUDA(cudaHostAlloc(&ctx->h_fence, sizeof(SlotCnt) * HICR_MAX_SLOTS, cudaHostAllocDefault));
     INIT_CUDA(cudaHostAlloc(&ctx->h_call, sizeof(CallResult) * 4, cudaHostAllocMapped));
     memset(ctx->h_call, 0, sizeof(CallResult) * 4);
     INIT_CUDA(cudaHostGetDevicePointer(&ctx->d_call, ctx->h_call, 0));
@@ -214,13 +248,7 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
             return rc;
         }
     }
-    {
-        // host threads for host-resident tables: the caller's plus helpers
-        int threads = 4;
-        const char *e = getenv("HICR_STAGE_THREADS");
-        if (e && *e) threads = std::max(1, std::min(64, atoi(e)));
-        ctx->stage_pool = stage_pool_create(threads - 1);
-    }
+    ctx->stage_pool = stage_pool_create(kStageThreads - 1);   // host threads for host-resident tables, beside the caller's
     *out = ctx;
     return HICR_OK;
 }
@@ -230,14 +258,10 @@ int hicr_finalize(hicr_ctx_t *ctx)
     if (!ctx) return HICR_ERR_INVALID_ARG;
     (void)cudaSetDevice(ctx->device);
     (void)cudaStreamSynchronize(ctx->stream);
-#ifdef HICR_TRACE
-    if (getenv("HICR_TRACE_FILE")) trace_dump(getenv("HICR_TRACE_FILE"));
-#endif
     stage_pool_destroy(ctx->stage_pool);
     stage_done_free(ctx->stage_done);
     cudaFree(ctx->d_slots);
-    cudaFree(ctx->d_sent);
-    cudaFree(ctx->d_recv);
+    cudaFree(ctx->d_cnt);
     cudaFree(ctx->d_ctl);
     cudaFree(ctx->d_chunk);
     for (auto *v : {&ctx->free_stage, &ctx->used_stage})
@@ -259,7 +283,7 @@ int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_
 {
     if (!ctx || !out) return HICR_ERR_INVALID_ARG;
     if (!dev_ptr && size) return HICR_ERR_INVALID_ARG;
-    if (size == kInvalidSize) return HICR_ERR_INVALID_ARG;
+    if (size > kSizeMask) return HICR_ERR_INVALID_ARG;
     if (dev_ptr) {
         // "If the communication manager supports communication between the memory spaces
         // ... Otherwise, it will be rejected": only this device's memory.
@@ -272,39 +296,36 @@ int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_
         if (a.type != cudaMemoryTypeDevice || a.device != ctx->device) return HICR_ERR_UNSUPPORTED_SPACE;
         if ((uint64_t)(uintptr_t)dev_ptr + size < (uint64_t)(uintptr_t)dev_ptr) return HICR_ERR_INVALID_ARG;
     }
-    if (ctx->slots.size() >= HICR_MAX_SLOTS) return HICR_ERR_NO_CAPACITY;
-    SlotRow row{(uint64_t)(uintptr_t)dev_ptr, size};
-    const size_t id = ctx->slots.size();
-    // ordered after everything already enqueued on the stream; the row lives in pageable
-    // host memory, so the runtime stages it before returning
-    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + id, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
-    ctx->slots.push_back(row);
-    ctx->sent.push_back(0);
-    ctx->recv.push_back(0);
-    ctx->ring_refs.push_back(0);
-    ctx->registered_bytes += size;
-    *out = (hicr_slot_t)id;
-    return HICR_OK;
+    return slot_install(ctx, (uint64_t)(uintptr_t)dev_ptr, size, 0, out);
 }
 
 int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
-    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    if (ctx->ring_refs[slot]) return HICR_ERR_BUSY;
-    SlotRow row{0, kInvalidSize};
-    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + slot, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
-    ctx->registered_bytes -= ctx->slots[slot].size;
-    ctx->slots[slot] = row;
+    const int64_t i = slot_find(ctx, slot);
+    if (i < 0) return HICR_ERR_INVALID_SLOT;
+    if (ctx->ring_refs[i]) return HICR_ERR_BUSY;
+    const SlotRow row{0, kInvalidMeta};
+    HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + i, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->registered_bytes -= row_size(ctx->rows[i]);
+    ctx->rows[i] = row;
+    ctx->push_stale = true;
+    // the index can be handed out again under the next generation (ids kept from before then name
+    // nothing); an index that has used up its generations is retired
+    if (ctx->gen[i] < kMaxGen) {
+        auto &f = ctx->free_idx;
+        f.insert(std::upper_bound(f.begin(), f.end(), (uint32_t)i, std::greater<uint32_t>()), (uint32_t)i);
+    }
     return HICR_OK;
 }
 
 int hicr_slot_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64_t *recv)
 {
     if (!ctx || !sent || !recv) return HICR_ERR_INVALID_ARG;
-    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    *sent = ctx->sent[slot];
-    *recv = ctx->recv[slot];
+    const int64_t i = slot_find(ctx, slot);
+    if (i < 0) return HICR_ERR_INVALID_SLOT;
+    *sent = ctx->cnt[i].sent;
+    *recv = ctx->cnt[i].recv;
     return HICR_OK;
 }
 
@@ -348,18 +369,21 @@ int hicr_fence_async(hicr_ctx_t *ctx)
 int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64_t recv)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
-    if (slot >= ctx->slots.size() || ctx->slots[slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    auto reached = [&] { return ctx->sent[slot] >= sent && ctx->recv[slot] >= recv; };
+    const int64_t si = slot_find(ctx, slot);
+    if (si < 0) return HICR_ERR_INVALID_SLOT;
+    SlotCnt &c = ctx->cnt[si];
+    auto reached = [&] { return c.sent >= sent && c.recv >= recv; };
     if (reached()) return HICR_OK;
     if (!ctx->epoch_open || ctx->batches_in_epoch == 0) return HICR_ERR_INVALID_ARG;   // nothing outstanding: never
-    if (slot < kPushSlots && ctx->slots.size() <= kPushSlots) {
+    if (!ctx->push_stale && (uint64_t)si < ctx->last_n_push) {
         // Every batch pushes the cumulative counters next to its completion record when its
         // copies are complete and visible: four flagged words per slot.  A snapshot whose four
         // flags agree comes from one batch; counters only grow, so the first such snapshot that
         // reaches the expected counts ends the wait.
-        const unsigned long long *w = ctx->h_rec[kRecRing].w + (size_t)slot * kPushWordsPerSlot;
+        const unsigned long long *w = ctx->h_rec[kRecRing].w + (size_t)si * kPushWordsPerSlot;
         const unsigned long long *last = ctx->h_rec[ctx->batches_in_epoch - 1].w;
         const uint32_t last_flag = rec_flag(ctx->batch_seq);
+        const uint64_t lo_seq = std::max(ctx->born[si], ctx->batch_seq - ctx->batches_in_epoch);
         unsigned spins = 0;
         for (;;) {
             uint32_t lf = 0;
@@ -367,11 +391,14 @@ int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64
             unsigned long long v[kPushWordsPerSlot];
             for (int k = 0; k < kPushWordsPerSlot; k++) v[k] = *reinterpret_cast<const volatile unsigned long long *>(w + k);
             const uint32_t f = (uint32_t)(v[0] >> 32);
-            if (f != 0 && (uint32_t)(v[1] >> 32) == f && (uint32_t)(v[2] >> 32) == f && (uint32_t)(v[3] >> 32) == f) {
+            // ... and from a batch of this epoch launched after the slot took the index
+            bool ours = false;
+            for (uint64_t q = ctx->batch_seq; q > lo_seq && !ours; q--) ours = f == rec_flag(q);
+            if (ours && (uint32_t)(v[1] >> 32) == f && (uint32_t)(v[2] >> 32) == f && (uint32_t)(v[3] >> 32) == f) {
                 const uint64_t sv = join64((uint32_t)v[0], (uint32_t)v[1]), rv = join64((uint32_t)v[2], (uint32_t)v[3]);
-                if (sv >= ctx->sent[slot] && rv >= ctx->recv[slot]) {
-                    ctx->sent[slot] = sv;
-                    ctx->recv[slot] = rv;
+                if (sv >= c.sent && rv >= c.recv) {
+                    c.sent = sv;
+                    c.recv = rv;
                 }
                 if (reached()) return HICR_OK;
             }

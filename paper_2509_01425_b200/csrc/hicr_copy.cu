@@ -50,26 +50,6 @@ __device__ __forceinline__ unsigned long long globaltimer()
     return t;
 }
 
-#ifdef HICR_TRACE
-// debug build only (_work probes): per-CTA %globaltimer stamps of the last batch
-__device__ unsigned long long g_trace[8 * 1024];
-#define TRACE(k) do { if (tid == 0 && blockIdx.x < 1024) g_trace[blockIdx.x * 8 + (k)] = globaltimer(); } while (0)
-void trace_dump(const char *path)
-{
-    static unsigned long long h[8 * 1024];
-    if (cudaMemcpyFromSymbol(h, g_trace, sizeof(h)) != cudaSuccess) return;
-    FILE *f = fopen(path, "w");
-    if (!f) return;
-    for (int b = 0; b < 1024; b++) {
-        if (!h[b * 8]) continue;
-        for (int k = 0; k < 8; k++) fprintf(f, "%llu%c", h[b * 8 + k], k == 7 ? '\n' : ' ');
-    }
-    fclose(f);
-}
-#else
-#define TRACE(k) do { } while (0)
-#endif
-
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned *p)
 {
     unsigned v;
@@ -129,16 +109,11 @@ struct EngineArgs {
     Ctl *ctl;
     WorkItem *chunk_q;
     uint64_t chunk_cap;
-    unsigned long long *sent;
-    unsigned long long *recv;
+    SlotCnt *cnt;                    // [HICR_MAX_SLOTS] cumulative message counters
     unsigned long long *rec;         // this batch's record words (device alias of mapped pinned memory)
     unsigned long long *push;        // [kPushWordsPerSlot * kPushSlots] pushed counter words (mapped pinned memory)
     uint32_t n_push;
     uint32_t flag;                   // rec_flag(sequence number of this batch)
-    uint32_t gss;                    // guided self-scheduling divisor: ticket = left / (gss x warps)
-    uint32_t max_group;              // units per warp ticket, at most (<= kMaxGroup)
-    uint32_t min_group;              // ... and at least
-    uint32_t prefetch;               // descriptors per warp whose source is prefetched into L2 before the barrier
     uint32_t skip_barrier;           // the host validated the table and it holds no large descriptor
     uint32_t hand_out;               // kHandOutVote (device tables), or what the host's own count says
 };
@@ -157,7 +132,7 @@ __device__ __forceinline__ SlotRow slot_row(const SlotRow *cache, const SlotRow 
     const uint4 v = __ldg(reinterpret_cast<const uint4 *>(global + s));
     SlotRow r;
     r.base = (uint64_t)v.x | ((uint64_t)v.y << 32);
-    r.size = (uint64_t)v.z | ((uint64_t)v.w << 32);
+    r.meta = (uint64_t)v.z | ((uint64_t)v.w << 32);
     return r;
 }
 
@@ -171,25 +146,24 @@ __device__ __forceinline__ void load_desc_raw(const hicr_desc_t *d, uint4 &lo, u
                  : "l"(reinterpret_cast<const unsigned char *>(d) + 16));
 }
 
-// Check one descriptor (its 32 bytes in lo, hi) against the slot table: destination before source,
-// overflow-safe "off + size <= slot size".  Returns 0 or the error id; on success src/dst
-// are absolute addresses.
+// Check one descriptor (its 32 bytes in lo, hi) against the slot table with THE validator
+// (check_transfer, hicr_internal.cuh).  Returns 0 or the error id; on success src/dst are
+// absolute addresses and ds/ss the table indices of the two slots.
 __device__ __forceinline__ unsigned resolve(const uint4 &lo, const uint4 &hi, const SlotRow *cache,
                                             const SlotRow *global, uint32_t n_slots, uint32_t &ds, uint32_t &ss,
                                             uint64_t &dst, uint64_t &src, uint64_t &size)
 {
-    ds = lo.x;
-    ss = lo.y;
+    ds = lo.x & kSlotIndexMask;
+    ss = lo.y & kSlotIndexMask;
     const uint64_t dst_off = (uint64_t)lo.z | ((uint64_t)lo.w << 32);
     const uint64_t src_off = (uint64_t)hi.x | ((uint64_t)hi.y << 32);
     size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
-    SlotRow dr{0, kInvalidSize}, sr{0, kInvalidSize};
-    if (ds < n_slots) dr = slot_row(cache, global, n_slots, ds);
-    if (ss < n_slots) sr = slot_row(cache, global, n_slots, ss);
-    if (dr.size == kInvalidSize) return kBadInvalidSlot;
-    if (dst_off > dr.size || size > dr.size - dst_off) return kBadOutOfBounds;
-    if (sr.size == kInvalidSize) return kBadInvalidSlot;
-    if (src_off > sr.size || size > sr.size - src_off) return kBadOutOfBounds;
+    SlotRow dr{0, kInvalidMeta}, sr{0, kInvalidMeta};
+    const bool d_in = ds < n_slots, s_in = ss < n_slots;
+    if (d_in) dr = slot_row(cache, global, n_slots, ds);
+    if (s_in) sr = slot_row(cache, global, n_slots, ss);
+    const unsigned bad = check_transfer(dr, d_in, lo.x, dst_off, sr, s_in, lo.y, src_off, size);
+    if (bad) return bad;
     dst = dr.base + dst_off;
     src = sr.base + src_off;
     return 0;
@@ -202,8 +176,8 @@ __device__ __forceinline__ unsigned resolve_small(const uint4 &lo, const uint4 &
 {
     const uint64_t size = (uint64_t)hi.z | ((uint64_t)hi.w << 32);
     if (size == 0 || size > kSmallMax) return 0;
-    dst = slot_row(cache, global, n_slots, lo.x).base + ((uint64_t)lo.z | ((uint64_t)lo.w << 32));
-    src = slot_row(cache, global, n_slots, lo.y).base + ((uint64_t)hi.x | ((uint64_t)hi.y << 32));
+    dst = slot_row(cache, global, n_slots, lo.x & kSlotIndexMask).base + ((uint64_t)lo.z | ((uint64_t)lo.w << 32));
+    src = slot_row(cache, global, n_slots, lo.y & kSlotIndexMask).base + ((uint64_t)hi.x | ((uint64_t)hi.y << 32));
     return (unsigned)size;
 }
 
@@ -237,7 +211,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     const uint32_t n_slots = a.n_slots;
     const bool use_hist = n_slots <= kSmemSlotHist;
     if (blockIdx.x == 0 && tid == 0) ctl->t_start = globaltimer();
-    TRACE(0);
     // the first tile's descriptors are requested before anything else, so that their DRAM
     // round trip overlaps the slot-table fetch and the shared-memory set-up
     uint4 alo = make_uint4(0, 0, 0, 0), ahi = alo;
@@ -247,7 +220,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         for (uint32_t i = tid; i < n_slots; i += kThreads) {
             const uint4 v = __ldg(reinterpret_cast<const uint4 *>(a.slots + i));
             cache[i].base = (uint64_t)v.x | ((uint64_t)v.y << 32);
-            cache[i].size = (uint64_t)v.z | ((uint64_t)v.w << 32);
+            cache[i].meta = (uint64_t)v.z | ((uint64_t)v.w << 32);
         }
     if (use_hist)
         for (uint32_t i = tid; i < 2 * n_slots; i += kThreads) hist[i] = 0;
@@ -268,9 +241,8 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // descriptors [g c0, (g+1) c0)); the others are atomics on a shared cursor that counts
     // from the end of the static tickets.
     const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
-    const unsigned gdiv = a.gss * nw, gmax = a.max_group;
-    const unsigned gmin = a.min_group;
-    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, gmin), gmax); };
+    const unsigned gdiv = kGss * nw;
+    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, 1u), kMaxGroup); };
     // (a multiple of 8 when it can be: team-sized descriptors are copied 8 at a time)
     const unsigned cnt_static0 = ticket_size(n, 0), cnt_static = cnt_static0 >= 8 ? cnt_static0 & ~7u : cnt_static0;
     const unsigned static_end = nw * cnt_static;
@@ -371,7 +343,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     if (fhave) load_desc_raw(a.descs + first0 + lane, flo, fhi);
 
     // ================================================================ grid barrier
-    TRACE(1);
     uint64_t src = 0, dst = 0;
     unsigned sz32 = 0;
     if (fhave) {
@@ -399,7 +370,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         // barrier is through, and reading a source range that passed its own checks has no
         // effect if the batch is rejected.  Issued AFTER the arrival: a release waits for the
         // prefetches in flight before it.
-        unsigned pm = __ballot_sync(0xffffffffu, sz32 != 0 && (unsigned)lane < a.prefetch);
+        unsigned pm = __ballot_sync(0xffffffffu, sz32 != 0 && (unsigned)lane < kPrefetchDescs);
         while (pm) {
             const int l = __ffs(pm) - 1;
             pm &= pm - 1;
@@ -417,14 +388,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     }
     const bool ok = ((sync >> kSyncBadShift) & kSyncFieldMask) == 0;
     if (blockIdx.x == 0 && tid == 0) ctl->t_mid = globaltimer();
-    TRACE(2);
 
     if (ok) {
         // ============================================================ counters (a6)
         if (use_hist) {
             for (uint32_t s = tid; s < 2 * n_slots; s += kThreads) {
                 const unsigned v = hist[s];
-                if (v) atomicAdd(s < n_slots ? &a.sent[s] : &a.recv[s - n_slots], (unsigned long long)v);
+                if (v) atomicAdd(s < n_slots ? &a.cnt[s].sent : &a.cnt[s - n_slots].recv, (unsigned long long)v);
             }
         } else {
             // slot table too large for the shared-memory histogram: count straight into the
@@ -434,13 +404,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
                 uint32_t ss = 0xffffffffu, ds = 0xffffffffu;
                 if (i < a.n) {
                     const uint4 lo = __ldg(reinterpret_cast<const uint4 *>(a.descs + i));
-                    ds = lo.x;
-                    ss = lo.y;
+                    ds = lo.x & kSlotIndexMask;
+                    ss = lo.y & kSlotIndexMask;
                 }
                 const unsigned ms = __match_any_sync(0xffffffffu, ss);
-                if (i < a.n && lane == __ffs(ms) - 1) atomicAdd(&a.sent[ss], (unsigned long long)__popc(ms));
+                if (i < a.n && lane == __ffs(ms) - 1) atomicAdd(&a.cnt[ss].sent, (unsigned long long)__popc(ms));
                 const unsigned md = __match_any_sync(0xffffffffu, ds);
-                if (i < a.n && lane == __ffs(md) - 1) atomicAdd(&a.recv[ds], (unsigned long long)__popc(md));
+                if (i < a.n && lane == __ffs(md) - 1) atomicAdd(&a.cnt[ds].recv, (unsigned long long)__popc(md));
             }
         }
 
@@ -499,7 +469,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         // 1 KiB copy.)  Three tickets are in flight per warp: k is
         // being copied, the descriptors of k+1 are being loaded, the atomic of k+2 is on its
         // way, so neither latency is exposed between two copies.
-        TRACE(3);
         first1 = sh_first1 + warp * cnt1;
         // Team-sized descriptors (the CTAs' votes, or the host's own count) are latency-bound, not
         // bandwidth-bound: equal counts are balanced enough, and 2368 warps drawing tickets from
@@ -571,22 +540,19 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             nhave = (unsigned)lane < cnt1 && first1 + lane < n;
             if (nhave) load_desc_raw(a.descs + first1 + lane, nlo, nhi);
         }
-        TRACE(4);
         if (lane == 0) tma_drain(tma);
     }
 
     // ================================================================ finish (feeds a7)
     __syncthreads();
-    TRACE(5);
     if (tid == 0) sh_flag = atom_inc_acq_rel_u32(&ctl->done) == gridDim.x - 1;
     __syncthreads();
-    TRACE(6);
     if (!sh_flag) return;
     // last CTA: every CTA's copies and counter updates are complete and visible on the device
     // (release increments above, acquired by this CTA's thread 0 and handed on by the barrier).
     // Publish the cumulative counters and the completion record as flagged 8-byte words.
     for (uint32_t s = tid; s < a.n_push; s += kThreads) {
-        const unsigned long long sv = __ldcg(&a.sent[s]), rv = __ldcg(&a.recv[s]);
+        const unsigned long long sv = __ldcg(&a.cnt[s].sent), rv = __ldcg(&a.cnt[s].recv);
         unsigned long long *w = a.push + (size_t)s * kPushWordsPerSlot;
         put_word(w + 0, (uint32_t)sv, a.flag);
         put_word(w + 1, (uint32_t)(sv >> 32), a.flag);
@@ -669,22 +635,11 @@ int engine_setup(hicr_ctx *ctx)
                                                                  engine_smem_bytes(kSmemSlotHist)));
     if (per_sm < 1) return HICR_ERR_NO_CAPACITY;
     per_sm = std::min(per_sm, kCtasPerSm);
-    // tuning overrides (experiments only; the defaults are what is measured and tested)
+    // HICR_TMA_MIN: smallest 16 B-aligned chunk that takes the bulk-copy path (0xffffffff = never).
+    // The one tuning knob left; tests run the large-descriptor cases with the path forced on and off.
     const char *e = getenv("HICR_TMA_MIN");
     if (e && *e) ctx->tma_min = (uint32_t)strtoul(e, nullptr, 0);
     if (ctx->tma_min < 16) ctx->tma_min = 16;
-    e = getenv("HICR_CTAS_PER_SM");
-    if (e && *e) per_sm = std::max(1, std::min(per_sm, atoi(e)));
-    e = getenv("HICR_GSS");
-    if (e && *e) ctx->gss = (uint32_t)std::max(1, atoi(e));
-    e = getenv("HICR_MAX_GROUP");
-    if (e && *e) ctx->max_group = (uint32_t)std::max(1, std::min((int)kMaxGroup, atoi(e)));
-    e = getenv("HICR_MIN_GROUP");
-    if (e && *e) ctx->min_group = (uint32_t)std::max(1, std::min((int)ctx->max_group, atoi(e)));
-    e = getenv("HICR_ZERO_COPY");
-    if (e && *e) ctx->zero_copy_descs = strtoull(e, nullptr, 0);
-    e = getenv("HICR_PREFETCH");
-    if (e && *e) ctx->prefetch = (uint32_t)std::max(0, std::min(32, atoi(e)));
     ctx->engine_grid = (int)std::min<unsigned>(ctx->num_sms * per_sm, kMaxGrid);
     return HICR_OK;
 }
@@ -701,6 +656,15 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     if (n >= (1ull << 31)) return HICR_ERR_NO_CAPACITY;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
 
+    // before anything of this batch is staged: an epoch that has used up its completion records
+    // drains them (and recycles the staging blocks of the batches that are then complete)
+    if (ctx->batches_in_epoch == kRecRing) {
+        int rc = drain_epoch(ctx, false);
+        if (rc != HICR_OK) return rc;
+    }
+    int rc = ensure_queues(ctx, n);
+    if (rc != HICR_OK) return rc;
+
     uint64_t units = ~0ull;   // work tickets of the copy phase, when the host knows them
     const hicr_desc_t *d_descs = descs;
     bool skip_barrier = false;
@@ -712,50 +676,43 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         // A bad descriptor leaves earlier pieces in the staging block, which nothing reads: no
         // kernel is launched.
         StageBlock b;
-        int rc = get_stage(ctx, n * sizeof(hicr_desc_t), &b);
+        rc = get_stage(ctx, n * sizeof(hicr_desc_t), &b);
         if (rc != HICR_OK) return rc;
         uint64_t ns = 0, nc = 0, small_bytes = 0;
-        rc = stage_table(ctx, descs, n, b, first_bad, &nc, &ns, &small_bytes);
+        int bad_status = HICR_OK;
+        rc = stage_table(ctx, descs, n, b, first_bad, &bad_status, &nc, &ns, &small_bytes);
+        if (rc == HICR_OK && bad_status != HICR_OK) rc = bad_status;
         if (rc != HICR_OK) {
+            // earlier pieces of the table may be on their way to b.dev: the block is reusable once they
+            // have landed (the error path is not a hot one)
+            (void)cudaStreamSynchronize(ctx->stream);
             ctx->free_stage.push_back(b);
             return rc;
         }
         units = nc + (ns + kWarps - 1) / kWarps;
         ctx->used_stage.push_back(b);
         // pinned staging is device-accessible under unified addressing: short tables stay there
-        d_descs = static_cast<const hicr_desc_t *>(n <= ctx->zero_copy_descs ? b.host : b.dev);
+        d_descs = static_cast<const hicr_desc_t *>(n <= kZeroCopyDescs ? b.host : b.dev);
         // checked against the host mirror of the slot table, which the device copy follows in
         // stream order: with no chunk queue to wait for either, the kernel needs no barrier
         skip_barrier = nc == 0;
         hand_out = ns && small_bytes <= kTeamMax * ns ? kHandOutStatic : kHandOutDynamic;
     }
 
-    if (ctx->batches_in_epoch == kRecRing) {
-        int rc = drain_epoch(ctx, false);
-        if (rc != HICR_OK) return rc;
-    }
-    int rc = ensure_queues(ctx, n);
-    if (rc != HICR_OK) return rc;
-
     EngineArgs a;
     a.descs = d_descs;
     a.n = n;
     a.slots = ctx->d_slots;
-    a.n_slots = (uint32_t)ctx->slots.size();
+    a.n_slots = (uint32_t)ctx->rows.size();
     a.tma_min = ctx->tma_min;
     a.ctl = ctx->d_ctl;
     a.chunk_q = ctx->d_chunk;
     a.chunk_cap = ctx->chunk_cap;
-    a.sent = ctx->d_sent;
-    a.recv = ctx->d_recv;
+    a.cnt = ctx->d_cnt;
     a.rec = ctx->d_rec[ctx->batches_in_epoch].w;
     a.push = ctx->d_rec[kRecRing].w;
     a.n_push = std::min<uint32_t>(a.n_slots, kPushSlots);
     a.flag = rec_flag(ctx->batch_seq + 1);
-    a.gss = ctx->gss;
-    a.max_group = ctx->max_group;
-    a.min_group = ctx->min_group;
-    a.prefetch = ctx->prefetch;
     a.skip_barrier = skip_barrier ? 1u : 0u;
     a.hand_out = hand_out;
 
@@ -774,5 +731,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     ctx->batch_seq++;
     ctx->batches_in_epoch++;
     ctx->epoch_open = true;
+    ctx->last_n_push = a.n_push;
+    ctx->push_stale = false;
     return HICR_OK;
 }

@@ -19,7 +19,7 @@ namespace hicr {
 // 0 < size <= kSmallMax : copied in place from the descriptor table, warp per descriptor (a4)
 // size >  kSmallMax     : split at kChunkBytes-aligned destination addresses, CTA-per-chunk queue (a5)
 constexpr uint64_t kSmallMax = 8192;
-constexpr uint64_t kChunkBytes = 131072;   // 32 KiB: 5765 GB/s on config 3a, 64 KiB: 5990, 128 KiB: 6118 (fewer CTA barriers and tickets per byte)
+constexpr uint64_t kChunkBytes = 131072;   // 128 KiB.  Config 3a: 32 KiB chunks 5765 GB/s, 64 KiB 5990, 128 KiB 6118 (fewer CTA barriers and tickets per byte)
 constexpr int kThreads = 256;              // 8 warps per CTA of the engine kernel
 constexpr int kWarps = kThreads / 32;
 constexpr int kCtasPerSm = 2;              // persistent grid = SMs x kCtasPerSm; 16 warps x 4 x 16 B x 32 lanes = 32 KiB of
@@ -39,17 +39,71 @@ constexpr unsigned kTeamMax = 16 * kTeam * kTeamVecs;   // descriptors up to thi
 constexpr uint64_t kZeroCopyDescs = 1024;   // host tables up to this many descriptors are read by the kernel straight from
                                             // pinned staging (32 KiB over PCIe costs less than enqueueing a copy: ~1.5 vs ~5 us)
 constexpr unsigned kMaxGroup = 32;         // units per warp ticket, at most (one per lane)
+constexpr unsigned kGss = 3;               // guided self-scheduling: a warp ticket is 1 / (kGss x warps) of what is left
+constexpr unsigned kPrefetchDescs = 2;     // descriptors per warp whose source goes to L2 while the grid barrier fills
+constexpr int kStageThreads = 4;           // host threads that check and stage a host-resident table (caller included)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
-constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3;
+constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3, kBadDirection = 4;
+
+// A slot id is {generation:20 | table index:12}.  Unregistering frees the index; the next
+// registration that takes it bumps the generation, so an id kept from before names nothing.
+constexpr int kSlotIndexBits = 12;
+constexpr uint32_t kSlotIndexMask = (1u << kSlotIndexBits) - 1;
+static_assert((1u << kSlotIndexBits) == HICR_MAX_SLOTS, "slot index field covers the table");
 
 // One row of the device slot table: "minimum information required to describe a segment
 // of memory (e.g., size, starting address)".
+//   meta = {remote:1 | global:1 | generation:18 | size:44}; all ones = not registered.
+// global = a Global Memory Slot; remote = its storage belongs to another
+// instance (base is then a peer-mapped address).
 struct SlotRow {
     uint64_t base;
-    uint64_t size;   // kInvalidSize = not registered
+    uint64_t meta;
 };
-constexpr uint64_t kInvalidSize = ~0ull;
+constexpr int kSizeBits = 44, kGenBits = 18;
+constexpr uint64_t kSizeMask = (1ull << kSizeBits) - 1;          // slots of up to 16 TiB - 1
+constexpr uint64_t kGenMask = (1ull << kGenBits) - 1;
+constexpr uint64_t kRowGlobal = 1ull << 62, kRowRemote = 1ull << 63;
+constexpr uint64_t kInvalidMeta = ~0ull;
+constexpr uint32_t kMaxGen = (uint32_t)kGenMask - 1;             // an index whose generation reaches this is retired
+
+// Per-slot message counters, cumulative since registration (reading 7).
+struct SlotCnt {
+    unsigned long long sent, recv;
+};
+
+__host__ __device__ inline uint64_t row_size(const SlotRow &r) { return r.meta & kSizeMask; }
+__host__ __device__ inline uint32_t row_gen(const SlotRow &r) { return (uint32_t)((r.meta >> kSizeBits) & kGenMask); }
+__host__ __device__ inline uint64_t row_meta(uint64_t size, uint32_t gen, uint64_t flags)
+{
+    return size | ((uint64_t)gen << kSizeBits) | flags;
+}
+
+// (a2) THE validator, used by the engine kernel for device-resident tables and by the host
+// threads for host-resident ones: one end of a transfer against its slot row.  `in_table` =
+// the id's index lies inside the table.  Overflow-safe "off + size <= slot size".
+__host__ __device__ inline unsigned check_end(const SlotRow &r, bool in_table, uint32_t id, uint64_t off, uint64_t size)
+{
+    if (!in_table || r.meta == kInvalidMeta || row_gen(r) != (id >> kSlotIndexBits)) return kBadInvalidSlot;
+    const uint64_t sz = row_size(r);
+    if (off > sz || size > sz - off) return kBadOutOfBounds;
+    return 0;
+}
+// Whole descriptor: destination before source, then the direction rule -- Local-to-Local,
+// Local-to-Global and Global-to-Local are allowed, "Global-to-Global operations are not
+// permitted".
+__host__ __device__ inline unsigned check_transfer(const SlotRow &dr, bool d_in, uint32_t d_id, uint64_t d_off,
+                                                   const SlotRow &sr, bool s_in, uint32_t s_id, uint64_t s_off,
+                                                   uint64_t size)
+{
+    unsigned bad = check_end(dr, d_in, d_id, d_off, size);
+    if (bad) return bad;
+    bad = check_end(sr, s_in, s_id, s_off, size);
+    if (bad) return bad;
+    if (dr.meta & sr.meta & kRowGlobal) return kBadDirection;
+    return 0;
+}
 
 // Item of the chunk queue (32 B so that one lane fetches it with two 16 B loads).
 struct __align__(16) WorkItem {
@@ -95,7 +149,7 @@ static_assert(sizeof(Ctl) == 640, "Ctl is five 128-byte lines");
 // and polled by hicr_fence.  Every 8-byte word is {low: 32 bits of payload, high: flag},
 // flag = rec_flag(batch sequence number) != 0.  A naturally aligned 8-byte store is
 // single-copy atomic, so a word whose flag matches carries its payload: no system-scope
-// fence orders the words (each one costs about 1.6 us on the way out, _work/rtbench).
+// fence orders the words (each one costs about 1.6 us on the way out, S5.1).
 constexpr int kRecWords = 16;
 enum RecWord { kRwBadLo = 0, kRwBadHi, kRwNChunk, kRwTStartLo, kRwTStartHi, kRwTMidLo, kRwTMidHi, kRwTEndLo, kRwTEndHi,
                kRwUsed };
@@ -471,11 +525,9 @@ struct StageBlock {
     size_t bytes = 0;
 };
 
-}  // namespace hicr
-
-namespace hicr {
 class StagePool;
-}
+
+}  // namespace hicr
 
 struct hicr_ctx {
     int device = 0;
@@ -483,13 +535,16 @@ struct hicr_ctx {
     int num_sms = 0;
     std::string cuda_error;
 
-    // slot table: host mirror + device copy
-    std::vector<hicr::SlotRow> slots;        // size = ids handed out so far
-    std::vector<uint64_t> sent, recv;        // host mirror, refreshed at fence / channel calls
+    // slot table: host mirror + device copy.  rows.size() = high-water mark of indices handed
+    // out; a freed index keeps its generation in `gen` and waits in `free_idx` (lowest first).
+    std::vector<hicr::SlotRow> rows;         // meta == kInvalidMeta: not registered
+    std::vector<uint32_t> gen;               // generation of the current (or last) registration of the index
+    std::vector<uint32_t> free_idx;          // freed indices, kept sorted descending (back() = lowest)
+    std::vector<hicr::SlotCnt> cnt;          // host mirror of the counters, refreshed at fence / channel calls
+    std::vector<uint64_t> born;              // batch_seq when the index was last handed out (older snapshots are not its)
     std::vector<uint32_t> ring_refs;         // live channels using the slot as ring
     hicr::SlotRow *d_slots = nullptr;        // [HICR_MAX_SLOTS]
-    unsigned long long *d_sent = nullptr;    // [HICR_MAX_SLOTS]
-    unsigned long long *d_recv = nullptr;    // [HICR_MAX_SLOTS]
+    hicr::SlotCnt *d_cnt = nullptr;          // [HICR_MAX_SLOTS]
     uint64_t registered_bytes = 0;
 
     // engine control block (device, self-cleaning) and per-batch completion records
@@ -505,6 +560,9 @@ struct hicr_ctx {
     uint64_t epoch_error_batch = 0, epoch_error_index = 0;
     int last_error = HICR_OK;                // of the last fence, for hicr_fence_error
     uint64_t last_error_batch = 0, last_error_index = 0;
+    uint32_t last_n_push = 0;                // slots whose counters the last launched batch pushes beside its record
+    bool push_stale = true;                  // the pushed snapshot of the last batch does not cover everything the mirror
+                                             // must show (a channel kernel ran after it, the table changed, ...)
 
     // chunk queue (large descriptors expanded by the binning phase)
     hicr::WorkItem *d_chunk = nullptr;
@@ -513,14 +571,13 @@ struct hicr_ctx {
     // staging of host-resident descriptor tables (returned to `free_stage` at the fence)
     std::vector<hicr::StageBlock> free_stage, used_stage;
 
-    // host threads that check and stage host-resident tables (HICR_STAGE_THREADS, default 4 incl. the caller)
+    // host threads that check and stage host-resident tables (kStageThreads, the caller included)
     hicr::StagePool *stage_pool = nullptr;
     std::atomic<uint64_t> *stage_done = nullptr;
     uint64_t stage_done_cap = 0;
 
-    // counter read-back for slot tables larger than kPushSlots (pinned)
-    unsigned char *h_fence = nullptr;
-    size_t h_fence_bytes = 0;
+    // counter read-back (pinned): the whole table, for fences the pushed snapshot does not serve
+    hicr::SlotCnt *h_fence = nullptr;
 
     // host-call channel results (mapped pinned)
     hicr::CallResult *h_call = nullptr;
@@ -530,11 +587,6 @@ struct hicr_ctx {
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
     uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
-    uint32_t gss = 3;                        // HICR_GSS: guided self-scheduling divisor of the warp tickets
-    uint32_t max_group = hicr::kMaxGroup;    // HICR_MAX_GROUP: units per warp ticket, at most
-    uint64_t zero_copy_descs = hicr::kZeroCopyDescs;   // HICR_ZERO_COPY: host tables up to this long are read in place
-    uint32_t min_group = 1;                  // HICR_MIN_GROUP: units per warp ticket, at least
-    uint32_t prefetch = 2;                   // HICR_PREFETCH: descriptors per warp whose source goes to L2 before the barrier
 
     bool profiling = false;
     cudaEvent_t ev[2] = {nullptr, nullptr};
@@ -549,15 +601,24 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what);
 int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
 int engine_setup(hicr_ctx *ctx);
-int check_desc(const hicr_desc_t &d, const SlotRow *rows, size_t nslots);
 int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const StageBlock &b, uint64_t *first_bad,
-                uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
+                int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
+int bad_to_status(unsigned id);
+int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hicr_slot_t *out);
 StagePool *stage_pool_create(int helpers);
 void stage_pool_destroy(StagePool *p);
 void stage_done_free(std::atomic<uint64_t> *p);
-#ifdef HICR_TRACE
-void trace_dump(const char *path);
-#endif
+
+// Table index of a live slot id, or -1 (unknown index, unregistered, or an id from an earlier
+// registration of the index).
+inline int64_t slot_find(const hicr_ctx *ctx, hicr_slot_t id)
+{
+    const uint32_t i = id & kSlotIndexMask;
+    if (i >= ctx->rows.size()) return -1;
+    const SlotRow &r = ctx->rows[i];
+    if (r.meta == kInvalidMeta || row_gen(r) != (id >> kSlotIndexBits)) return -1;
+    return (int64_t)i;
+}
 }  // namespace hicr
 
 #define HICR_CUDA(ctx, call)                                                   \

@@ -4,7 +4,7 @@
 //
 // One pass over a 2 MiB table is bound by host memory bandwidth (a plain memcpy of it takes
 // as long as check + copy on one core of the GPU box), so the table is cut into pieces that
-// the caller's thread and kHelpers helper threads claim from a shared cursor.  CUDA calls
+// the caller's thread and kStageThreads - 1 helper threads claim from a shared cursor.  CUDA calls
 // stay on the caller's thread: it sends every finished prefix of pieces to the device while
 // the others are still being checked.  Helpers spin for a short while after a job (a loop of
 // batches finds them awake) and then sleep on a condition variable.
@@ -29,13 +29,15 @@ struct StageJob {
     std::atomic<uint64_t> large{0}, small{0}, small_bytes{0};
 };
 
-int check_desc(const hicr_desc_t &d, const SlotRow *rows, size_t nslots)
+// One descriptor against the host mirror of the slot table, with THE validator the engine
+// kernel uses for device-resident tables (check_transfer, hicr_internal.cuh).  0 or an error id.
+static inline unsigned check_desc(const hicr_desc_t &d, const SlotRow *rows, size_t nslots)
 {
-    if (d.dst_slot >= nslots || rows[d.dst_slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    if (d.dst_off > rows[d.dst_slot].size || d.size > rows[d.dst_slot].size - d.dst_off) return HICR_ERR_OUT_OF_BOUNDS;
-    if (d.src_slot >= nslots || rows[d.src_slot].size == kInvalidSize) return HICR_ERR_INVALID_SLOT;
-    if (d.src_off > rows[d.src_slot].size || d.size > rows[d.src_slot].size - d.src_off) return HICR_ERR_OUT_OF_BOUNDS;
-    return HICR_OK;
+    const uint32_t di = d.dst_slot & kSlotIndexMask, si = d.src_slot & kSlotIndexMask;
+    const bool d_in = di < nslots, s_in = si < nslots;
+    static const SlotRow none{0, kInvalidMeta};
+    return check_transfer(d_in ? rows[di] : none, d_in, d.dst_slot, d.dst_off, s_in ? rows[si] : none, s_in, d.src_slot,
+                          d.src_off, d.size);
 }
 
 // Claim one piece and do it; false if none is left.  A piece with a bad descriptor is marked
@@ -48,7 +50,7 @@ static bool work_one(StageJob &j)
     uint64_t state = 1, nc = 0, ns = 0, sb = 0;
     for (uint64_t i = i0; i < i1; i++) {
         const hicr_desc_t d = j.in[i];
-        if (check_desc(d, j.rows, j.n_slots) != HICR_OK) {
+        if (check_desc(d, j.rows, j.n_slots) != 0) {
             state = 2;
             break;
         }
@@ -97,10 +99,12 @@ public:
             cv_.notify_all();
         }
     }
+    // Store-buffering pattern with the helper's { active_++ ; job_.load }: both sides are
+    // sequentially consistent, so either the helper sees nullptr or finish() sees it active.
     void finish()
     {
-        job_.store(nullptr, std::memory_order_release);
-        while (active_.load(std::memory_order_acquire) != 0) std::this_thread::yield();
+        job_.store(nullptr, std::memory_order_seq_cst);
+        while (active_.load(std::memory_order_seq_cst) != 0) std::this_thread::yield();
     }
 
 private:
@@ -123,8 +127,8 @@ private:
                 }
             }
             seen = epoch_.load(std::memory_order_acquire);
-            active_.fetch_add(1, std::memory_order_acq_rel);
-            StageJob *j = job_.load(std::memory_order_acquire);
+            active_.fetch_add(1, std::memory_order_seq_cst);
+            StageJob *j = job_.load(std::memory_order_seq_cst);
             if (j) work(*j);
             active_.fetch_sub(1, std::memory_order_acq_rel);
         }
@@ -140,10 +144,11 @@ private:
 };
 
 // (a2) for a host table: check + stage `descs` into the pinned block `b`, send it to b.dev on
-// the context's stream.  Returns HICR_OK, or the status of the lowest bad index (*first_bad)
-// with nothing launched.  Totals: chunk-queue bound, small descriptors and their bytes.
+// the context's stream.  Returns HICR_OK or a CUDA failure; *bad_status = HICR_OK or the status of
+// the lowest bad index (*first_bad), with nothing to launch.  Totals: chunk-queue bound, small
+// descriptors and their bytes.
 int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const StageBlock &b, uint64_t *first_bad,
-                uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes)
+                int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes)
 {
     constexpr uint64_t kPiece = 4096, kSendPieces = 4;
     StageJob j;
@@ -152,8 +157,8 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
     j.n = n;
     j.piece = kPiece;
     j.n_pieces = (n + kPiece - 1) / kPiece;
-    j.rows = ctx->slots.data();
-    j.n_slots = ctx->slots.size();
+    j.rows = ctx->rows.data();
+    j.n_slots = ctx->rows.size();
     if (ctx->stage_done_cap < j.n_pieces) {
         delete[] ctx->stage_done;
         ctx->stage_done = new std::atomic<uint64_t>[j.n_pieces];
@@ -165,6 +170,7 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
     if (parallel) ctx->stage_pool->start(&j);
 
     int rc = HICR_OK;
+    *bad_status = HICR_OK;
     uint64_t sent = 0, ready = 0;   // pieces sent to the device / checked prefix
     while (sent < j.n_pieces) {
         const bool worked = work_one(j);
@@ -174,16 +180,19 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
             if (st == 2) {
                 // every earlier piece is clean, so the lowest bad index of the table is in here
                 const uint64_t i0 = ready * kPiece, i1 = std::min(n, i0 + kPiece);
-                for (uint64_t i = i0; i < i1 && rc == HICR_OK; i++) {
-                    rc = check_desc(descs[i], j.rows, j.n_slots);
-                    if (rc != HICR_OK && first_bad) *first_bad = i;
+                for (uint64_t i = i0; i < i1 && *bad_status == HICR_OK; i++) {
+                    const unsigned bad = check_desc(descs[i], j.rows, j.n_slots);
+                    if (bad) {
+                        *bad_status = bad_to_status(bad);
+                        if (first_bad) *first_bad = i;
+                    }
                 }
                 break;
             }
             ready++;
         }
-        if (rc != HICR_OK) break;
-        if (n <= ctx->zero_copy_descs) {
+        if (rc != HICR_OK || *bad_status != HICR_OK) break;
+        if (n <= kZeroCopyDescs) {
             sent = ready;   // short table: the kernel reads the pinned staging block in place (no copy to enqueue)
         } else if (ready - sent >= kSendPieces || (ready == j.n_pieces && ready > sent)) {
             const uint64_t i0 = sent * kPiece, i1 = std::min(n, ready * kPiece);
@@ -198,7 +207,7 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
             std::this_thread::yield();   // the helpers hold the remaining pieces
         }
     }
-    if (rc != HICR_OK) j.next.store(j.n_pieces, std::memory_order_relaxed);   // nobody claims any more
+    if (rc != HICR_OK || *bad_status != HICR_OK) j.next.store(j.n_pieces, std::memory_order_relaxed);   // nobody claims any more
     if (parallel) ctx->stage_pool->finish();
     *n_chunk_bound = j.large.load();
     *n_small = j.small.load();

@@ -28,6 +28,20 @@ def _ctx(hicr):
     return hicr.Context(0, torch.cuda.current_stream().cuda_stream)
 
 
+def fence_counters_both(ctx, o, ids, what=""):
+    """The kernels' own message counters (device memory), not the host mirror the channel calls
+    keep: one zero-size descriptor (moves nothing, counts one message, reading 4) as a device
+    batch + hicr_fence on the GPU, the same on the oracle, then every slot's counters.  The
+    fence reads what the device counted (reading 15: one message per token)."""
+    d = W.make_descs([ids[0]], [ids[-1]], [0], [0], [0])
+    assert o.memcpy_batch(d)[0] == oracle.OK and o.fence() == oracle.OK
+    t = torch.from_numpy(d.view(np.uint8).copy()).cuda()
+    ctx.memcpy_batch(t, n=1)
+    ctx.fence()
+    for s in ids:
+        assert ctx.slot_counters(s) == o.slot_counters(s), "%s device counters of slot %d" % (what, s)
+
+
 class Pair:
     """The same ring / source / sink set up on the oracle and on the GPU."""
 
@@ -53,6 +67,7 @@ class Pair:
             assert t.cpu().numpy().tobytes() == a.tobytes(), "%s %s differs" % (what, name)
         for s in self.ids:
             assert self.ctx.slot_counters(s) == self.o.slot_counters(s), "%s counters of slot %d" % (what, s)
+        fence_counters_both(self.ctx, self.o, self.ids, what)
 
     def close(self):
         self.ctx.close()
@@ -244,6 +259,7 @@ def _mpsc_both(hicr, w, max_batch):
             assert g_r[p].cpu().numpy().tobytes() == rings[p].tobytes(), "ring %d" % p
         for s in rid + sid + kid:
             assert ctx.slot_counters(s) == o.slot_counters(s)
+        fence_counters_both(ctx, o, rid + sid + kid, "mpsc")
 
 
 @pytest.mark.parametrize("P,N,T,C,maxb", [(1, 5000, 64, 16, 16), (5, 3000, 8, 32, 48), (148, 20000, 64, 1024, 256),
@@ -255,7 +271,107 @@ def test_mpsc_stream(hicr, P, N, T, C, maxb):
     _mpsc_both(hicr, w, maxb)
 
 
+@pytest.mark.parametrize("P,N1,N2,T,C,maxb", [(3, 1000, 777, 64, 48, 20), (148, 1500, 1100, 64, 1024, 256), (7, 10, 5, 24, 16, 3)])
+def test_mpsc_stream_twice_continues_counters(hicr, P, N1, N2, T, C, maxb):
+    """Two hicr_mpsc_stream runs on one channel set with N1 % C != 0: heads and tails keep
+    counting (monotone indices), so the second run's first token goes to ring
+    position N1 mod C, as the oracle's does.  Sources and sinks at non-zero offsets (the second
+    run continues where the first stopped).  Ring images, head / tail, sinks and counters equal
+    the oracle's after each run."""
+    assert N1 % C != 0
+    rng = np.random.default_rng(P * 131 + C)
+    lead = 16 * int(rng.integers(1, 9))                    # sources start `lead` bytes into their slots
+    srcs = [rng.integers(0, 256, lead + (N1 + N2) * T, dtype=np.uint8) for _ in range(P)]
+    o = Oracle()
+    rings = [np.zeros(T * C, dtype=np.uint8) for _ in range(P)]
+    sinks = [np.zeros((N1 + N2) * T + 32, dtype=np.uint8) for _ in range(P)]
+    rid = [o.slot_register(a) for a in rings]
+    sid = [o.slot_register(a) for a in srcs]
+    kid = [o.slot_register(a) for a in sinks]
+    chs = [o.channel_create(rid[p], T, C)[1] for p in range(P)]
+
+    def oracle_run(first, count):
+        for p in range(P):
+            done = 0
+            while done < count:
+                rc, k = o.channel_push(chs[p], sid[p], lead + (first + done) * T, min(count - done, maxb))
+                assert rc == oracle.OK and k > 0
+                assert o.channel_pop(chs[p], kid[p], 32 + (first + done) * T, C) == (oracle.OK, k)
+                done += k
+
+    with _ctx(hicr) as ctx:
+        g_r = [torch.from_numpy(a.copy()).cuda() for a in rings]
+        g_s = [torch.from_numpy(a).cuda() for a in srcs]
+        g_k = [torch.from_numpy(a.copy()).cuda() for a in sinks]
+        assert [ctx.slot_register(t) for t in g_r + g_s + g_k] == rid + sid + kid
+        m = ctx.mpsc_create(rid, T, C)
+        for first, count in ((0, N1), (N1, N2)):
+            oracle_run(first, count)
+            m.stream(sid, kid, count, maxb, src_offs=[lead + first * T] * P, dst_offs=[32 + first * T] * P)
+            torch.cuda.synchronize()
+            for p in range(P):
+                assert m.counters(p) == o.channel_counters(chs[p]) == (first + count, first + count)
+                assert g_k[p].cpu().numpy().tobytes() == sinks[p].tobytes(), "sink %d after %d" % (p, first + count)
+                assert g_r[p].cpu().numpy().tobytes() == rings[p].tobytes(), "ring %d after %d" % (p, first + count)
+            for s in rid + sid + kid:
+                assert ctx.slot_counters(s) == o.slot_counters(s)
+            fence_counters_both(ctx, o, rid + sid + kid, "mpsc run ending at %d" % (first + count))
+
+
+def test_batch_then_channel_calls_then_fence(hicr):
+    """memcpy_batch; channel_push / pop; fence on one context: the fence must report the batch's
+    messages AND the channel's (the channel kernels count on the device after the batch's
+    snapshot of the counters was taken).  Then the other order."""
+    T, C = 32, 8
+    rng = np.random.default_rng(5)
+    p = Pair(hicr, T, C, rng.integers(0, 256, 40 * T, dtype=np.uint8), 40 * T)
+    try:
+        d = W.make_descs([p.ids[2]] * 3, [p.ids[1]] * 3, [600, 700, 800], [0, 64, 128], [64, 50, 1])
+        t = torch.from_numpy(d.view(np.uint8).copy()).cuda()
+        for order in (0, 1):
+            if order == 0:
+                assert p.o.memcpy_batch(d)[0] == oracle.OK
+                p.ctx.memcpy_batch(t, n=len(d))
+            for _ in range(3):
+                assert p.ch.push(p.ids[1], 0, 5) == p.o.channel_push(p.och, p.ids[1], 0, 5)[1] == 5
+                assert p.ch.pop(p.ids[2], 0, 8) == p.o.channel_pop(p.och, p.ids[2], 0, 8)[1] == 5
+            if order == 1:
+                assert p.o.memcpy_batch(d)[0] == oracle.OK
+                p.ctx.memcpy_batch(t, n=len(d))
+            assert p.o.fence() == oracle.OK
+            p.ctx.fence()
+            for s in p.ids:
+                assert p.ctx.slot_counters(s) == p.o.slot_counters(s), "order %d slot %d" % (order, s)
+        p.check("batch + channel + fence")
+    finally:
+        p.close()
+
+
 # ------------------------------------------------------------ full-size configs 5a / 5b
+@pytest.mark.timeout(1200)
+def test_config5a_full_size_host_calls(hicr):
+    """BASELINE.json config 5a exactly as worded -- "each push followed by a consumer pop of the
+    available tokens" -- at FULL size (2^24 tokens of 256 B, capacity 1024, ~32.7 k batches)
+    through hicr_channel_push / hicr_channel_pop, one launch per call: every returned count,
+    then sink, ring, head / tail and message counters against the oracle's same call sequence."""
+    w = W.spsc()
+    assert w.n_tokens == 1 << 24 and w.token_bytes == 256 and w.capacity == 1024
+    p = Pair(hicr, w.token_bytes, w.capacity, w.source_image(0), w.n_tokens * w.token_bytes)
+    try:
+        _oracle_spsc(p, w)
+        pos = 0
+        for b in w.batches[0]:
+            b = int(b)
+            assert p.ch.push(p.ids[1], pos * p.T, b) == b
+            assert p.ch.pop(p.ids[2], pos * p.T, p.C) == b
+            pos += b
+        assert pos == 1 << 24 and p.ch.counters() == (1 << 24, 1 << 24)
+        p.check("5a full size, host calls")
+    finally:
+        p.close()
+
+
+
 @pytest.mark.timeout(900)
 def test_config5a_full_size_stream(hicr):
     """BASELINE.json config 5a at FULL size (2^24 tokens of 256 B, capacity 1024, batches
@@ -338,6 +454,7 @@ def test_pingpong_capacity_one(hicr, s):
         assert imgs[3].tobytes() == imgs[2].tobytes()
         for i in ids:
             assert ctx.slot_counters(i) == o.slot_counters(i)
+        fence_counters_both(ctx, o, ids, "ping-pong")
 
 
 # ------------------------------------------------------------ locking MPSC
@@ -400,6 +517,7 @@ def test_mpsc_locking(hicr, P, N, T, C, maxb):
         assert ch.counters() == o.channel_counters(och) == (P * N, P * N)
         for s in [rid, kid] + sid:
             assert ctx.slot_counters(s) == o.slot_counters(s)
+        fence_counters_both(ctx, o, [rid, kid] + sid, "locking mpsc")
         # the channel keeps working through host calls afterwards, on the same counters
         assert ch.push(sid[0], 0, 1) == 1 and ch.pop(kid, 0, 1) == 1
         assert ch.counters() == (P * N + 1, P * N + 1)

@@ -161,6 +161,42 @@ def test_several_batches_one_fence(hicr, name):
     assert_same(w, ref, run_gpu(w, split=100, device_tables=True))
 
 
+@pytest.mark.parametrize("name", ["tiny", "chain"])
+def test_host_tables_split_epochs(hicr, name):
+    """Configs 1 and 4 with every epoch cut into several HOST-table batches before its fence."""
+    w = SMALL[name]()
+    ref = run_oracle(w)
+    assert_same(w, ref, run_gpu(w, split=3))
+    assert_same(w, ref, run_gpu(w, split=9))
+
+
+def test_more_host_batches_than_completion_records(hicr):
+    """One epoch of 150 HOST-table batches of mixed sizes, among them tables of more than 1 MiB
+    between short ones (a short table is read from pinned staging in place, a long one is
+    copied): the epoch drains its 64 completion records twice while staging blocks are in use,
+    and no block may be recycled before the kernel that reads it has run."""
+    w = W.bulk_aligned(n_desc=150000, slot_bytes=256 * W.MiB, page=256, n_sets=1)
+    ref = run_oracle(w)
+    d = w.epochs[0]
+    rng = np.random.default_rng(11)
+    cuts, pos = [], 0
+    for k in range(149):
+        n = 40000 if k in (64, 65, 130) else int(rng.integers(1, 300))      # 40,000 x 32 B = 1.22 MiB
+        cuts.append((pos, pos + n))
+        pos += n
+    cuts.append((pos, len(d)))
+    assert pos < len(d)
+    with _ctx(hicr) as ctx:
+        bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(2)]
+        ids = [ctx.slot_register(b) for b in bufs]
+        for a, b in cuts:
+            ctx.memcpy_batch(np.ascontiguousarray(d[a:b]))
+        ctx.fence()
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == ref[0][s].tobytes(), "slot %d" % s
+        assert [ctx.slot_counters(i) for i in ids] == ref[1][-1]
+
+
 def test_config1_counters_golden_on_gpu(hicr, golden_dir):
     g = json.load(open(os.path.join(golden_dir, "config1_counters.json")))
     w = W.tiny()
@@ -278,6 +314,153 @@ def test_unregister_then_use_is_invalid_slot(hicr):
         assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
 
 
+def test_register_between_batch_and_fence(hicr):
+    """memcpy_batch; slot_register(new); fence: the batch pushed the counters of the slots that
+    existed at its launch, the fence must not wait for more, and the new slot reads (0, 0)."""
+    w = W.tiny()
+    ref = run_oracle(w)
+    with _ctx(hicr) as ctx:
+        bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(2)]
+        ids = [ctx.slot_register(b) for b in bufs]
+        t = to_device_table(w.epochs[0])
+        ctx.memcpy_batch(t, n=len(w.epochs[0]))
+        extra = torch.zeros(128, dtype=torch.uint8, device="cuda")
+        ie = ctx.slot_register(extra)
+        ctx.fence()
+        assert [ctx.slot_counters(i) for i in ids] == ref[1][-1]
+        assert ctx.slot_counters(ie) == (0, 0)
+        for s in range(2):
+            assert bufs[s].cpu().numpy().tobytes() == ref[0][s].tobytes()
+        # and hicr_fence_expected after a registration falls back to the full read-back
+        ctx.memcpy_batch(t, n=len(w.epochs[0]))
+        ie2 = ctx.slot_register(torch.zeros(16, dtype=torch.uint8, device="cuda"))
+        ctx.fence_expected(ids[1], 0, 2 * len(w.epochs[0]))
+        assert ctx.slot_counters(ids[1]) == (0, 2 * len(w.epochs[0])) and ctx.slot_counters(ie2) == (0, 0)
+        ctx.fence()
+
+
+def test_slot_ids_are_recycled_under_a_new_generation(hicr):
+    """Unregistering frees the table index; the next registration takes it under a new id, with
+    zeroed counters, and the old id names nothing any more.  A context is not
+    capped at HICR_MAX_SLOTS registrations over its lifetime."""
+    with _ctx(hicr) as ctx:
+        a = torch.arange(64, dtype=torch.uint8, device="cuda")
+        b = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        ia, ib = ctx.slot_register(a), ctx.slot_register(b)
+        assert (ia, ib) == (0, 1)
+        ctx.memcpy_batch(W.make_descs([ib], [ia], [0], [0], [8]))
+        ctx.fence()
+        assert ctx.slot_counters(ib) == (0, 1)
+        ctx.slot_unregister(ib)
+        c = torch.zeros(64, dtype=torch.uint8, device="cuda")
+        ic = ctx.slot_register(c)
+        assert ic != ib and ic & 0xfff == ib                       # same index, next generation
+        assert ctx.slot_counters(ic) == (0, 0)                      # counters restart at registration
+        for table in (False, True):                                 # the old id is dead, on the host and on the device
+            d = W.make_descs([ib], [ia], [8], [8], [8])
+            with pytest.raises(hicr.HicrError) as e:
+                if table:
+                    t = to_device_table(d)
+                    ctx.memcpy_batch(t, n=1)
+                    ctx.fence()
+                else:
+                    ctx.memcpy_batch(d)
+            assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+        with pytest.raises(hicr.HicrError):
+            ctx.slot_counters(ib)
+        t = to_device_table(W.make_descs([ic, ic], [ia, ia], [0, 16], [32, 0], [16, 5]))
+        ctx.memcpy_batch(t, n=2)
+        ctx.fence()
+        assert ctx.slot_counters(ic) == (0, 2) and ctx.slot_counters(ia) == (3, 0)
+        assert c.cpu().tolist()[:21] == list(range(32, 48)) + list(range(5))
+        assert b.cpu().tolist()[:8] == list(range(8)) and sum(b.cpu().tolist()[8:]) == 0
+        # far more registrations than table rows over the context's lifetime
+        last = None
+        for k in range(hicr.HICR_MAX_SLOTS + 100):
+            last = ctx.slot_register(b)
+            ctx.slot_unregister(last)
+        assert last >> 12 >= 1000
+        ctx.memcpy_batch(W.make_descs([ic], [ia], [40], [0], [4]))
+        ctx.fence()
+        assert ctx.slot_counters(ic) == (0, 3)
+
+
+def test_visible_from_another_stream_after_fence(hicr):
+    """hicr_fence returns when the last CTA's completion record arrives; the kernel may still be
+    running its last instructions.  What the fence promises (hicr.h) must then hold for ANY
+    reader: a device-to-host copy and a kernel on OTHER streams, issued right after the fence
+    returned, see every byte of the epoch (S5.1 says why).  1,000 rounds of config 1's
+    descriptors from four rotating source images (so every round changes the destination bytes),
+    the context on a stream of its own."""
+    w = W.tiny()
+    sa, sb, sc = torch.cuda.Stream(), torch.cuda.Stream(), torch.cuda.Stream()
+    with torch.cuda.stream(sa):
+        ctx = hicr.Context(0, sa.cuda_stream)
+    try:
+        rng = np.random.default_rng(3)
+        src_imgs = [rng.integers(0, 256, w.slot_sizes[0], dtype=np.uint8) for _ in range(4)]
+        exp = []
+        from oracle import Oracle
+        for img in src_imgs:
+            o = Oracle()
+            dst = w.slot_image(1)
+            o.slot_register(img.copy())
+            o.slot_register(dst)
+            assert o.memcpy_batch(w.epochs[0])[0] == 0 and o.fence() == 0
+            exp.append(torch.from_numpy(dst.copy()).cuda())
+        with torch.cuda.stream(sa):
+            srcs = [torch.from_numpy(i).cuda() for i in src_imgs]
+            dst0 = torch.from_numpy(w.slot_image(1)).cuda()
+            dst = dst0.clone()
+            ids = [ctx.slot_register(t) for t in srcs]
+            idd = ctx.slot_register(dst)
+            tabs = []
+            for i in ids:
+                d = w.epochs[0].copy()
+                d["src_slot"], d["dst_slot"] = i, idd
+                tabs.append(to_device_table(d))
+        host = torch.empty(dst.numel(), dtype=torch.uint8).pin_memory()
+        flag = torch.zeros(1, dtype=torch.int32, device="cuda")
+        torch.cuda.synchronize()
+        n = len(w.epochs[0])
+        for r in range(1000):
+            k = r % 4
+            ctx.memcpy_batch(tabs[k], n=n)
+            ctx.fence()
+            # no synchronisation with stream A beyond the fence having returned
+            with torch.cuda.stream(sb):
+                host.copy_(dst, non_blocking=True)
+            with torch.cuda.stream(sc):
+                flag += (dst != exp[k]).any().to(torch.int32)
+            sb.synchronize()
+            assert torch.equal(host, exp[k].cpu()), "round %d: copy on another stream saw stale bytes" % r
+        sc.synchronize()
+        assert int(flag.item()) == 0, "a kernel on another stream saw stale bytes"
+    finally:
+        with torch.cuda.stream(sa):
+            ctx.close()
+
+
+def test_tma_min_knob(hicr, monkeypatch):
+    """HICR_TMA_MIN, the one tuning knob (read at hicr_init): the large-descriptor cases with
+    the bulk-copy path forced on for every aligned chunk and switched off altogether."""
+    w = W.heavy_tailed("a", n_slots=6, slot_bytes=16 * W.MiB, src_zone=2 * W.MiB, n_desc=2500, smax=2 * W.MiB, seed=77)
+    # make a good share of the large descriptors 16 B-congruent so that the bulk path carries them
+    d = w.epochs[0]
+    zone = w.meta["src_zone"]
+    new = d["src_off"] // 16 * 16 + d["dst_off"] % 16
+    new = np.where(new + d["size"] > zone, new - 16, new)
+    move = (d["size"] > 8192) & (d["size"] <= zone - 32) & (new >= 0) & (new + d["size"] <= zone)
+    d["src_off"][move] = new[move]
+    assert int(move.sum()) > 50
+    from oracle import hazard
+    assert hazard.check(d, w.slot_sizes) is None
+    ref = run_oracle(w)
+    for v in ("16", "0xffffffff"):
+        monkeypatch.setenv("HICR_TMA_MIN", v)
+        assert_same(w, ref, run_gpu(w, device_tables=True), "HICR_TMA_MIN=" + v)
+
+
 # ------------------------------------------------------------ full-size configs
 def test_config2_full_size(hicr):
     """BASELINE.json config 2 at full size (2 x 1 GiB, 4 x 65,536 x 4 KiB), in the launch
@@ -356,14 +539,16 @@ def test_chain_host_tables_static_hand_out(hicr):
 
 
 @pytest.mark.timeout(1800)
-def test_config3a_full_size(hicr):
-    """BASELINE.json config 3 (variant 3a, reading 19) at FULL size -- 64 slots x 256 MiB, 100,000
-    descriptors, one device-resident batch, one fence: the launch configuration bench.py times.
+@pytest.mark.parametrize("variant", ["a", "b"])
+def test_config3_full_size(hicr, variant):
+    """BASELINE.json config 3 (variants 3a and 3b, reading 19) at FULL size -- 64 slots x 256 MiB,
+    100,000 descriptors (3a) / every log-uniform draw that fits (3b), one device-resident batch, one
+    fence: the launch configuration bench.py times.
     The oracle gets the same descriptors one destination slot at a time, against slots trimmed
     to the zones they touch (the destination slot whole, every slot's 32 MiB source zone), so
     16 GiB never has to sit in host memory twice; every byte of every slot is compared."""
     from oracle import Oracle
-    w = W.heavy_tailed("a")
+    w = W.heavy_tailed(variant)
     d = w.epochs[0]
     zone = w.meta["src_zone"]
     n_slots = len(w.slot_sizes)

@@ -315,3 +315,21 @@ def test_chained_epochs_against_numpy_and_per_epoch_counters():
         lo, hi = p["dst_off"][order], (p["dst_off"] + p["size"])[order]
         j = np.searchsorted(lo, c["src_off"], side="right") - 1
         assert np.all(j >= 0) and np.all(c["src_off"] + c["size"] <= hi[j])
+
+
+def test_parallel_memcpy_baseline_equals_the_oracle():
+    """oracle/parallel_memcpy.c (bench.py's cpu_baseline_parallel: libc memcpy per descriptor on
+    all host cores) is a timing baseline, not the oracle; its image must still
+    be the oracle's on inputs that meet the epoch precondition, for 1 and for several threads."""
+    import workloads as W
+    for w in (W.heavy_tailed("a", n_slots=6, slot_bytes=4 * W.MiB, src_zone=W.MiB, n_desc=2000, smax=300000),
+              W.chained_epochs(n_epochs=1, n_desc=5000, slot_bytes=4 * W.MiB)):
+        ref = [w.slot_image(s) for s in range(len(w.slot_sizes))]
+        o = Oracle()
+        for a in ref:
+            o.slot_register(a)
+        assert o.memcpy_batch(w.epochs[0])[0] == oracle.OK
+        for threads in (1, 5):
+            got = [w.slot_image(s) for s in range(len(w.slot_sizes))]
+            oracle.parallel_memcpy_batch(got, w.epochs[0], threads)
+            assert all(a.tobytes() == b.tobytes() for a, b in zip(ref, got))
