@@ -28,6 +28,8 @@ ERR_INVALID_ARG = -1
 ERR_INVALID_SLOT = -2
 ERR_OUT_OF_BOUNDS = -3
 ERR_NO_CAPACITY = -5
+ERR_ILLEGAL_DIRECTION = -8   # "Global-to-Global operations are not permitted"
+ERR_DUPLICATE_KEY = -9       # a (tag, key) pair names one global slot; used by world.py
 
 # descriptor layout = the paper's argument order dst, dst_off, src, src_off, size
 DESC_DTYPE = np.dtype(
@@ -90,6 +92,9 @@ def _load():
     lib.oracle_free.restype = None
     lib.oracle_free.argtypes = [ctypes.c_void_p]
     lib.oracle_slot_register.argtypes = [ctypes.c_void_p, u8p, u64, P(u32)]
+    lib.oracle_slot_register_global.argtypes = [ctypes.c_void_p, ctypes.c_void_p, u32, P(u32)]
+    lib.oracle_slot_is_global.argtypes = [ctypes.c_void_p, u32]
+    lib.oracle_slot_global_counters.argtypes = [ctypes.c_void_p, u32, P(u64), P(u64)]
     lib.oracle_slot_unregister.argtypes = [ctypes.c_void_p, u32]
     lib.oracle_slot_counters.argtypes = [ctypes.c_void_p, u32, P(u64), P(u64)]
     lib.oracle_memcpy_batch.argtypes = [ctypes.c_void_p, ctypes.c_void_p, u64, P(u64)]
@@ -136,6 +141,27 @@ class Oracle:
 
     def slot_unregister(self, slot: int) -> int:
         return self._lib.oracle_slot_unregister(self._ctx, slot)
+
+    def slot_register_global(self, owner: "Oracle", owner_slot: int):
+        """This instance's view of the Global Memory Slot over ``owner``'s local slot.
+        Returns (status, slot id)."""
+        out = ctypes.c_uint32()
+        rc = self._lib.oracle_slot_register_global(self._ctx, owner._ctx, owner_slot, ctypes.byref(out))
+        if rc == OK and owner is not self:
+            self._keep.append(owner)          # the owner's storage outlives this view
+        return rc, (out.value if rc == OK else None)
+
+    def slot_is_global(self, slot: int) -> int:
+        """1 = Global Memory Slot, 0 = Local Memory Slot, negative = status."""
+        return self._lib.oracle_slot_is_global(self._ctx, slot)
+
+    def slot_global_counters(self, slot: int):
+        """Messages of all instances on the Global Memory Slot behind local slot ``slot`` (reading 23)."""
+        s, r = ctypes.c_uint64(), ctypes.c_uint64()
+        rc = self._lib.oracle_slot_global_counters(self._ctx, slot, ctypes.byref(s), ctypes.byref(r))
+        if rc != OK:
+            raise RuntimeError("oracle_slot_global_counters: %d" % rc)
+        return s.value, r.value
 
     def slot_counters(self, slot: int):
         s, r = ctypes.c_uint64(), ctypes.c_uint64()

@@ -34,6 +34,20 @@
  *                         printed examples.
  *   partial-push rule, zero-size rule, all-or-nothing errors: "parity unpinned" by the
  *                         paper (SURVEY S8(c) pts 4, 10, 12); fixed by unit tests.
+ *
+ * Global Memory Slots (S3.1.4): several oracle
+ * contexts stand for several HiCR instances in one process.  A Global Memory Slot is "a local
+ * memory slot ... made accessible to other HiCR instances": here a slot of
+ * kind GLOBAL in the table of every instance, over the storage of the volunteered local slot
+ * of its owner.  The collective exchange itself (who volunteers what under which tag and key)
+ * is oracle/world.py; this file holds the three legal directions -- "Global-to-Global
+ * operations are not permitted" -- and the counters.
+ *   oracle_slot_register_global / direction rule  pinned: the four slot-kind pairs of
+ *                         SPEC.md:78-84, the 2-instance put / get examples,
+ *                         a randomized copy graph against numpy slicing.
+ *   global counters (every message naming a global slot also counts at its owner, reading
+ *                         23 of DESIGN.md): "parity unpinned" by the paper; pinned to the
+ *                         closed form sum over instances of their own per-slot counts.
  */
 #include <stdint.h>
 #include <stdlib.h>
@@ -45,8 +59,11 @@ enum {
     ORC_ERR_INVALID_ARG = -1,
     ORC_ERR_INVALID_SLOT = -2,
     ORC_ERR_OUT_OF_BOUNDS = -3,
-    ORC_ERR_NO_CAPACITY = -5
+    ORC_ERR_NO_CAPACITY = -5,
+    ORC_ERR_ILLEGAL_DIRECTION = -8   /* "Global-to-Global operations are not permitted" */
 };
+
+struct orc_ctx_s;
 
 typedef struct {
     uint8_t *base;   /* starting address */
@@ -54,6 +71,13 @@ typedef struct {
     uint64_t sent;   /* messages sent from this slot, cumulative (reading 7) */
     uint64_t recv;   /* messages received into this slot, cumulative (reading 7) */
     int valid;
+    /* Global Memory Slot: the local slot `owner_slot` of instance `owner`, seen
+     * from this instance.  g_sent / g_recv of THAT local slot count the messages of all
+     * instances that named the global slot as source / destination (reading 23). */
+    int global;
+    struct orc_ctx_s *owner;
+    uint32_t owner_slot;
+    uint64_t g_sent, g_recv;
 } orc_slot;
 
 /* field order = the paper's call: dst, dst offset, src, src offset, size */
@@ -79,7 +103,7 @@ typedef struct {
     int valid;
 } orc_channel;
 
-typedef struct {
+typedef struct orc_ctx_s {
     orc_slot *slots;
     uint32_t n_slots, cap_slots;
     orc_pending *pending;
@@ -116,7 +140,53 @@ int oracle_slot_register(orc_ctx *o, uint8_t *ptr, uint64_t size, uint32_t *out)
     s->sent = 0;
     s->recv = 0;
     s->valid = 1;
+    s->global = 0;
+    s->owner = NULL;
+    s->owner_slot = 0;
+    s->g_sent = 0;
+    s->g_recv = 0;
     *out = o->n_slots++;
+    return ORC_OK;
+}
+
+/* One instance's view of a Global Memory Slot: the storage of local slot `owner_slot` of
+ * instance `owner` (which may be `o` itself), "made accessible to other HiCR instances"
+ * (PAPER.md:377).  Same size and starting address as the local slot behind it. */
+int oracle_slot_register_global(orc_ctx *o, orc_ctx *owner, uint32_t owner_slot, uint32_t *out)
+{
+    if (!o || !owner || !out) return ORC_ERR_INVALID_ARG;
+    if (owner_slot >= owner->n_slots || !owner->slots[owner_slot].valid) return ORC_ERR_INVALID_SLOT;
+    if (owner->slots[owner_slot].global) return ORC_ERR_INVALID_ARG;   /* only local slots are volunteered */
+    {
+        /* (o == owner: the table may move when it grows, so take the values first) */
+        uint8_t *base = owner->slots[owner_slot].base;
+        uint64_t size = owner->slots[owner_slot].size;
+        int rc = oracle_slot_register(o, base, size, out);
+        if (rc != ORC_OK) return rc;
+    }
+    o->slots[*out].global = 1;
+    o->slots[*out].owner = owner;
+    o->slots[*out].owner_slot = owner_slot;
+    return ORC_OK;
+}
+
+/* 1 if `slot` is this instance's view of a Global Memory Slot, 0 if it is a Local Memory Slot. */
+int oracle_slot_is_global(orc_ctx *o, uint32_t slot)
+{
+    if (!o) return ORC_ERR_INVALID_ARG;
+    if (slot >= o->n_slots || !o->slots[slot].valid) return ORC_ERR_INVALID_SLOT;
+    return o->slots[slot].global;
+}
+
+/* Messages of ALL instances that named the Global Memory Slot behind local slot `slot` of
+ * this instance as source (sent) / destination (recv); complete once every instance has
+ * fenced (reading 23). */
+int oracle_slot_global_counters(orc_ctx *o, uint32_t slot, uint64_t *sent, uint64_t *recv)
+{
+    if (!o || !sent || !recv) return ORC_ERR_INVALID_ARG;
+    if (slot >= o->n_slots || !o->slots[slot].valid) return ORC_ERR_INVALID_SLOT;
+    *sent = o->slots[slot].g_sent;
+    *recv = o->slots[slot].g_recv;
     return ORC_OK;
 }
 
@@ -194,6 +264,9 @@ int oracle_memcpy_batch(orc_ctx *o, const orc_desc *d, uint64_t n, uint64_t *fir
     for (k = 0; k < n; k++) {
         int rc = check_range(o, d[k].dst_slot, d[k].dst_off, d[k].size);
         if (rc == ORC_OK) rc = check_range(o, d[k].src_slot, d[k].src_off, d[k].size);
+        /* Local-to-Local, Local-to-Global and Global-to-Local only */
+        if (rc == ORC_OK && o->slots[d[k].dst_slot].global && o->slots[d[k].src_slot].global)
+            rc = ORC_ERR_ILLEGAL_DIRECTION;
         if (rc != ORC_OK) {
             if (first_bad) *first_bad = k;
             return rc;
@@ -217,8 +290,13 @@ int oracle_fence(orc_ctx *o)
     uint64_t k;
     if (!o) return ORC_ERR_INVALID_ARG;
     for (k = 0; k < o->n_pending; k++) {
-        o->slots[o->pending[k].src_slot].sent += 1;
-        o->slots[o->pending[k].dst_slot].recv += 1;
+        orc_slot *ss = &o->slots[o->pending[k].src_slot];
+        orc_slot *ds = &o->slots[o->pending[k].dst_slot];
+        ss->sent += 1;
+        ds->recv += 1;
+        /* a global slot's message also counts at its owner, on the local slot behind it */
+        if (ss->global) ss->owner->slots[ss->owner_slot].g_sent += 1;
+        if (ds->global) ds->owner->slots[ds->owner_slot].g_recv += 1;
     }
     o->n_pending = 0;
     return ORC_OK;

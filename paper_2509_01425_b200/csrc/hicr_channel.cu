@@ -42,6 +42,7 @@ struct hicr_mpsc {
     hicr::ChannelState *d_state = nullptr;   // [P]
     uint64_t *d_ptrs = nullptr;              // [4 * P] u64: ring base, source address, sink address, tokens before the run;
                                              // then [3 * P] u32: table indices of ring, source, sink
+    hicr::PipeRing *d_pipe = nullptr;        // [P] ring records of the bulk-copy pipeline (hicr_pipe.cu)
     std::vector<uint64_t> head, tail;
 };
 
@@ -66,61 +67,6 @@ __device__ __forceinline__ void ring_copy(unsigned char *ring, uint64_t ring_byt
         if (len > first) copy_span<U, kLdL2>(lin + first, ring, len - first, gtid, gsize);
     }
 }
-
-// ---- deep TMA ring of one driver lane: S stages of kTmaPiece bytes, up to S bulk loads in
-// flight ahead of the stores.  The single MPSC consumer has to keep far more bytes in flight
-// than its registers allow: 8 warps x 5 x 2 KiB = 80 KiB here against 16 KiB with 4 vectors
-// per lane.  kl / ks = loads / stores issued so far, ever: stage = k % S, mbarrier parity =
-// (k / S) & 1.
-template <int S, int PIECE>
-struct TmaRing {
-    unsigned char *stage;
-    uint64_t *bar;
-    unsigned kl, ks;
-};
-__device__ __forceinline__ void ring_wait_read(unsigned n)   // at most n of my bulk stores still read shared memory
-{
-    switch (n) {
-    case 0: bulk_wait_read<0>(); break;
-    case 1: bulk_wait_read<1>(); break;
-    case 2: bulk_wait_read<2>(); break;
-    case 3: bulk_wait_read<3>(); break;
-    case 4: bulk_wait_read<4>(); break;
-    default: bulk_wait_read<5>(); break;
-    }
-}
-// Driver lane only: dst[0, n) = src[0, n) in pieces of PIECE bytes; dst, src, n multiples of 16.
-// At most S - 1 loads run ahead of the stores, so the stage a load refills was handed to a
-// store at least one piece ago and the wait for that store's shared-memory read is short.
-// On return every load has landed (the source bytes have been read) and every store has been
-// issued, not necessarily completed.
-template <int S, int PIECE>
-__device__ __forceinline__ void tma_ring_copy(TmaRing<S, PIECE> &r, unsigned char *dst, const unsigned char *src, uint64_t n)
-{
-    static_assert(S >= 2 && S <= 7, "ring_wait_read covers up to 5 stores in flight");
-    const unsigned np = (unsigned)((n + PIECE - 1) / PIECE);
-    unsigned issued = 0, stored = 0;
-    while (stored < np) {
-        while (issued < np && r.kl - r.ks < (unsigned)(S - 1)) {
-            // the stage of load kl was last read by store kl - S; S - 1 - (kl - ks) stores came after it
-            if (r.kl >= (unsigned)S) ring_wait_read(S - 1 - (r.kl - r.ks));
-            const uint64_t off = (uint64_t)issued * PIECE;
-            const unsigned len = (unsigned)min((uint64_t)PIECE, n - off), st = r.kl % S;
-            mbar_expect_tx(r.bar + st, len);
-            bulk_g2s(r.stage + st * PIECE, src + off, len, r.bar + st);
-            r.kl++;
-            issued++;
-        }
-        const uint64_t off = (uint64_t)stored * PIECE;
-        const unsigned len = (unsigned)min((uint64_t)PIECE, n - off), st = r.ks % S;
-        mbar_wait(r.bar + st, (r.ks / S) & 1);
-        bulk_s2g(dst + off, r.stage + st * PIECE, len);
-        bulk_commit();
-        r.ks++;
-        stored++;
-    }
-}
-constexpr int kMpscStages = 3, kMpscPiece = 4096;   // 8 warps x 3 x 4 KiB = 96 KiB: two CTAs per SM stay co-resident
 
 // (a8) push / (a9) pop as one launch.  `lin` = the linear side (source slot for push,
 // destination slot for pop) already offset; lin_room = bytes available there.
@@ -260,10 +206,8 @@ spsc_stream_kernel(ChannelState *st, unsigned char *ring, uint64_t T, uint64_t C
 // the message counters.  head/tail keep counting from where the last run (or call) left them.
 __global__ void __launch_bounds__(kMpscThreads, 2)
 mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const uint64_t *__restrict__ ptrs,
-                   const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch, SlotCnt *cnt, int use_tma)
+                   const uint32_t *__restrict__ slot_ids, uint64_t tokens, uint64_t max_batch, SlotCnt *cnt)
 {
-    extern __shared__ __align__(128) unsigned char dyn_smem[];   // consumer, use_tma: [warp][stage][kMpscPiece]
-    __shared__ uint64_t bars[(kMpscThreads / 32) * kMpscStages];
     const uint64_t ring_bytes = C * T;
     const int tid = threadIdx.x;
     if (blockIdx.x < P) {
@@ -294,15 +238,6 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
     }
     // ---- the single consumer: warp w polls and drains rings w, w + nwarps, ...
     const int lane = tid & 31, warp = tid >> 5, nwarps = kMpscThreads / 32;
-    TmaRing<kMpscStages, kMpscPiece> tr;
-    tr.stage = dyn_smem + (size_t)warp * kMpscStages * kMpscPiece;
-    tr.bar = &bars[warp * kMpscStages];
-    tr.kl = tr.ks = 0;
-    if (use_tma && lane == 0) {
-        for (int i = 0; i < kMpscStages; i++) mbar_init(tr.bar + i, 1);
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-    }
-    __syncwarp();
     bool all_done = false;
     unsigned ns = 20;
     while (!all_done) {
@@ -326,18 +261,7 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
             unsigned char *ring = reinterpret_cast<unsigned char *>(ptrs[p]);
             // sink address of the token at ring count `tail`
             unsigned char *dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]) - (end - tokens) * T;
-            if (use_tma) {
-                // bulk copies ring -> shared -> sink, up to kMpscStages loads in flight; when the call
-                // returns the ring bytes have been read, so the tail can move while the stores drain
-                if (lane == 0) {
-                    fence_proxy_async();   // head was acquired in the generic proxy, the copies run in the async one
-                    const uint64_t rb = (tail % C) * T, len = k * T, a = min(len, ring_bytes - rb);
-                    tma_ring_copy<kMpscStages, kMpscPiece>(tr, dst + tail * T, ring + rb, a);
-                    if (len > a) tma_ring_copy<kMpscStages, kMpscPiece>(tr, dst + tail * T + a, ring, len - a);
-                }
-            } else {
-                ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
-            }
+            ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + tail * T, k * T, lane, 32);
             __syncwarp();
             if (lane == 0) {
                 st_release(&s->tail, tail + k);
@@ -351,7 +275,6 @@ mpsc_stream_kernel(ChannelState *st, uint32_t P, uint64_t T, uint64_t C, const u
         }
         if (!progressed && !all_done) backoff(ns); else ns = 20;
     }
-    if (use_tma && lane == 0) bulk_wait_all();   // the sink is complete (and shared memory free) before the CTA exits
 }
 
 // Device-resident LOCKING MPSC run ("locking, where a collective exclusive access
@@ -630,11 +553,28 @@ int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, h
         return HICR_ERR_OUT_OF_BOUNDS;
     if (total == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
-    int rc = channel_scratch(ch, n_batches * 8);
+    int rc = channel_scratch(ch, n_batches * 8 + sizeof(PipeRing));
     if (rc != HICR_OK) return rc;
     uint64_t *d_batches = reinterpret_cast<uint64_t *>(ch->d_tab);
     HICR_CUDA(ctx, cudaMemcpyAsync(d_batches, batch_tokens, n_batches * 8, cudaMemcpyHostToDevice, ctx->stream));
+    bool piped = false;
     {
+        // 16 B-aligned shapes: the pipeline of bulk copies (hicr_pipe.cu), many pieces in flight per end
+        PipeRing pr;
+        pr.st = ch->d_state;
+        pr.ring = reinterpret_cast<unsigned char *>(ctx->rows[ch->ring].base);
+        pr.src = reinterpret_cast<const unsigned char *>(ss.base + src_off);
+        pr.dst = reinterpret_cast<unsigned char *>(ds.base + dst_off);
+        pr.count0 = ch->head;
+        pr.id_ring = ch->ring;
+        pr.id_src = (uint32_t)si;
+        pr.id_dst = (uint32_t)di;
+        pr.pad = 0;
+        rc = pipe_run(ctx, &pr, reinterpret_cast<PipeRing *>(ch->d_tab + n_batches * 8), 1, ch->T, ch->C, total, d_batches, 0,
+                      ctx->d_call, &piped);
+        if (rc != HICR_OK) return rc;
+    }
+    if (!piped) {
         ChannelState *st = ch->d_state;
         unsigned char *ring = reinterpret_cast<unsigned char *>(ctx->rows[ch->ring].base);
         unsigned char *sp = reinterpret_cast<unsigned char *>(ss.base + src_off);
@@ -686,9 +626,11 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
     cudaError_t e = cudaMalloc(&m->d_state, sizeof(ChannelState) * producers);
     if (e == cudaSuccess) e = cudaMemsetAsync(m->d_state, 0, sizeof(ChannelState) * producers, ctx->stream);
     if (e == cudaSuccess) e = cudaMalloc(&m->d_ptrs, (size_t)producers * (4 * 8 + 3 * 4));
+    if (e == cudaSuccess) e = cudaMalloc(&m->d_pipe, (size_t)producers * sizeof(PipeRing));
     if (e != cudaSuccess) {
         cudaFree(m->d_state);
         cudaFree(m->d_ptrs);
+        cudaFree(m->d_pipe);
         delete m;
         return cuda_fail(ctx, e, "hicr_mpsc_create");
     }
@@ -703,6 +645,7 @@ int hicr_mpsc_destroy(hicr_mpsc_t *m)
     (void)cudaStreamSynchronize(m->ctx->stream);
     cudaFree(m->d_state);
     cudaFree(m->d_ptrs);
+    cudaFree(m->d_pipe);
     for (auto r : m->rings) m->ctx->ring_refs[r]--;
     delete m;
     return HICR_OK;
@@ -726,8 +669,6 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_
     if (N > (1ull << 48) / m->T) return HICR_ERR_OUT_OF_BOUNDS;
     std::vector<uint64_t> ptrs(4 * (size_t)P);
     std::vector<uint32_t> ids(3 * (size_t)P);
-    // every ring, sink and token size a multiple of 16 bytes: the consumer moves tokens with bulk copies
-    int use_tma = m->T % 16 == 0;
     for (uint32_t p = 0; p < P; p++) {
         const int64_t si = slot_find(ctx, src_slots[p]), di = slot_find(ctx, dst_slots[p]);
         if (si < 0 || di < 0) return HICR_ERR_INVALID_SLOT;
@@ -742,40 +683,50 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_
         ids[p] = m->rings[p];
         ids[P + p] = (uint32_t)si;
         ids[2 * P + p] = (uint32_t)di;
-        if ((ptrs[p] | ptrs[2 * P + p]) % 16) use_tma = 0;
     }
     if (N == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
-    // co-residency of all P + 1 CTAs is what makes the spin-waits safe
-    size_t smem = use_tma ? (size_t)(kMpscThreads / 32) * kMpscStages * kMpscPiece : 0;
-    int per_sm = 0;
-    if (use_tma) {
-        HICR_CUDA(ctx, cudaFuncSetAttribute(mpsc_stream_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, smem));
-        if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) {
-            use_tma = 0;
-            smem = 0;
+    // 16 B-aligned shapes: the pipeline of bulk copies (hicr_pipe.cu), one producer CTA and one consumer
+    // CTA per ring -- the single logical consumer is P CTAs
+    bool piped = false;
+    {
+        std::vector<PipeRing> pr(P);
+        for (uint32_t p = 0; p < P; p++) {
+            pr[p].st = m->d_state + p;
+            pr[p].ring = reinterpret_cast<unsigned char *>(ptrs[p]);
+            pr[p].src = reinterpret_cast<const unsigned char *>(ptrs[P + p]);
+            pr[p].dst = reinterpret_cast<unsigned char *>(ptrs[2 * P + p]);
+            pr[p].count0 = m->tail[p];
+            pr[p].id_ring = ids[p];
+            pr[p].id_src = ids[P + p];
+            pr[p].id_dst = ids[2 * P + p];
+            pr[p].pad = 0;
         }
+        int rc = pipe_run(ctx, pr.data(), m->d_pipe, P, m->T, m->C, N, nullptr, max_batch, nullptr, &piped);
+        if (rc != HICR_OK) return rc;
     }
-    if (!use_tma) {
+    if (!piped) {
+        // any other shape: vector copies, P producer CTAs and one consumer CTA whose warps share the rings;
+        // co-residency of all P + 1 CTAs is what makes the spin-waits safe
+        int per_sm = 0;
         HICR_CUDA(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, mpsc_stream_kernel, kMpscThreads, 0));
         if ((uint64_t)per_sm * ctx->num_sms < (uint64_t)P + 1) return HICR_ERR_NO_CAPACITY;
+        uint32_t *d_ids = reinterpret_cast<uint32_t *>(m->d_ptrs + 4 * (size_t)P);
+        // (pageable sources: the runtime stages them before returning)
+        HICR_CUDA(ctx, cudaMemcpyAsync(m->d_ptrs, ptrs.data(), ptrs.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
+        HICR_CUDA(ctx, cudaMemcpyAsync(d_ids, ids.data(), ids.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
+        ChannelState *st = m->d_state;
+        uint32_t Pv = P;
+        uint64_t T = m->T, C = m->C, tok = N, mb = max_batch;
+        const uint64_t *pp = m->d_ptrs;
+        const uint32_t *ip = d_ids;
+        SlotCnt *cnt = ctx->d_cnt;
+        void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &cnt};
+        HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_stream_kernel, dim3(P + 1), dim3(kMpscThreads), args, 0,
+                                                   ctx->stream));
+        ctx->launches++;
+        ctx->push_stale = true;
     }
-    uint32_t *d_ids = reinterpret_cast<uint32_t *>(m->d_ptrs + 4 * (size_t)P);
-    // (pageable sources: the runtime stages them before returning)
-    HICR_CUDA(ctx, cudaMemcpyAsync(m->d_ptrs, ptrs.data(), ptrs.size() * 8, cudaMemcpyHostToDevice, ctx->stream));
-    HICR_CUDA(ctx, cudaMemcpyAsync(d_ids, ids.data(), ids.size() * 4, cudaMemcpyHostToDevice, ctx->stream));
-    ChannelState *st = m->d_state;
-    uint32_t Pv = P;
-    uint64_t T = m->T, C = m->C, tok = N, mb = max_batch;
-    const uint64_t *pp = m->d_ptrs;
-    const uint32_t *ip = d_ids;
-    SlotCnt *cnt = ctx->d_cnt;
-    void *args[] = {&st, &Pv, &T, &C, &pp, &ip, &tok, &mb, &cnt, &use_tma};
-    HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)mpsc_stream_kernel, dim3(P + 1), dim3(kMpscThreads),
-                                               args, smem, ctx->stream));
-    ctx->launches++;
-    ctx->push_stale = true;
     HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
     for (uint32_t p = 0; p < P; p++) {
         m->head[p] += N;

@@ -171,6 +171,17 @@ struct __align__(128) ChannelState {
 };
 static_assert(sizeof(ChannelState) == 256, "ChannelState is two lines");
 
+// One ring of a device-resident pipeline run (hicr_pipe.cu): its counters, the ring slot, and where
+// the run's first token comes from and goes to.  count0 = head = tail at entry.
+struct PipeRing {
+    ChannelState *st;
+    unsigned char *ring;
+    const unsigned char *src;
+    unsigned char *dst;
+    unsigned long long count0;
+    uint32_t id_ring, id_src, id_dst, pad;   // table indices, for the message counters
+};
+
 // Result of one host-call push/pop, written by the kernel into mapped pinned memory.
 struct CallResult {
     unsigned long long k, head, tail;
@@ -605,6 +616,8 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
                 int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
 int bad_to_status(unsigned id);
 int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hicr_slot_t *out);
+int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t P, uint64_t T, uint64_t C, uint64_t tokens,
+             const uint64_t *d_batches, uint64_t max_batch, CallResult *res, bool *ran);
 StagePool *stage_pool_create(int helpers);
 void stage_pool_destroy(StagePool *p);
 void stage_done_free(std::atomic<uint64_t> *p);
