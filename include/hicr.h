@@ -41,6 +41,8 @@ extern "C" {
 #define HICR_ERR_BUSY             (-7)  /* object still referenced (e.g. slot used by a channel) */
 #define HICR_ERR_ILLEGAL_DIRECTION (-8) /* "Global-to-Global operations are not permitted"
                                                                                */
+#define HICR_ERR_DUPLICATE_KEY    (-9)  /* a (tag, key) pair names one global slot */
+#define HICR_ERR_TIMEOUT         (-10)  /* a global fence did not see the expected counts in time */
 
 typedef struct hicr_ctx hicr_ctx_t;          /* opaque context  */
 typedef struct hicr_channel hicr_channel_t;  /* opaque SPSC channel */
@@ -163,6 +165,85 @@ int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64
 /* After hicr_fence returned a deferred error: which batch of that epoch (0-based) and
  * which descriptor index in it was the first bad one.  Host pointers out (may be NULL). */
 int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad);
+
+/* ---- Global Memory Slots (S3.1.4) -------------
+ *
+ * "The communication manager also is in charge of creating and exchanging Global Memory Slots,
+ * local memory slots that are made accessible to other HiCR instances and can be used as the
+ * source or destination of distributed memcpy operations.  The exchange operation communicates
+ * the necessary metadata for remote instances to reach the associated memory slot."
+ * (PAPER.md:377).  An INSTANCE here is one context: one process per GPU (or several contexts of
+ * one process).  "The exchange of global memory slots is a collective operation: all instances
+ * must participate by volunteering zero or more local memory slots.  The operation returns as
+ * many global memory slots as the total amount of local memory slots exchanged.  Each of the
+ * resulting global memory slots are uniquely identified by a tag and key pair".
+ *
+ * The library has no transport of its own: the collective is split into its two LOCAL halves,
+ * and the caller carries the 256-byte handles between instances over whatever control plane it
+ * has (paper_2509_01425_b200/collective.py uses torch.distributed all_gather):
+ *   1. every instance calls hicr_global_volunteer once per local slot it volunteers;
+ *   2. the handles of ALL instances, in one order all instances agree on, go to
+ *      hicr_global_exchange on every instance, which returns one Global Memory Slot id per handle.
+ * A global slot id is an ordinary hicr_slot_t of this context: it names the owner's storage --
+ * the same address for the owner, a CUDA-IPC / peer mapping of it for every other instance, so a
+ * transfer runs in the initiator's copy kernels over NVLink ("the communication
+ * manager will use the accelerator-specific network to satisfy the request").  hicr_memcpy_batch
+ * takes it as source or destination: Local-to-Local, Local-to-Global (a put) and Global-to-Local
+ * (a get) are carried out, a descriptor with two global slots fails the batch with
+ * HICR_ERR_ILLEGAL_DIRECTION ("Global-to-Global operations are not permitted").
+ * Counters: a message on a global slot counts on the initiator's id like any other, and ALSO at
+ * the owner, on the local slot behind it (hicr_global_counters; reading 23). */
+#define HICR_GLOBAL_HANDLE_BYTES 256
+typedef struct hicr_global_handle {
+    unsigned char bytes[HICR_GLOBAL_HANDLE_BYTES];   /* opaque, position-independent, valid on this node */
+} hicr_global_handle_t;
+
+/* One line of a global fence's count exchange: what one instance has initiated so far on the
+ * global slot (tag, key), cumulative. */
+typedef struct hicr_global_count {
+    uint64_t tag, key, sent, recv;
+} hicr_global_count_t;
+
+/* Plumbing: which instance this context is (default 0 of 1).  Recorded in the handles. */
+int hicr_instance_set(hicr_ctx_t *ctx, uint32_t instance, uint32_t n_instances);
+
+/* Local half 1 of the exchange: describe the LOCAL slot `local_slot`, volunteered as (tag, key),
+ * in *out (host pointer).  HICR_ERR_INVALID_SLOT on an unknown id, HICR_ERR_INVALID_ARG if the
+ * slot is itself a global slot ("volunteering ... local memory slots"). */
+int hicr_global_volunteer(hicr_ctx_t *ctx, uint64_t tag, uint64_t key, hicr_slot_t local_slot,
+                          hicr_global_handle_t *out);
+
+/* Local half 2: `handles` (host pointer) = the n handles of all instances under `tag`, this
+ * context's own included; out_slots (host pointer, n ids) receives the Global Memory Slot of
+ * handles[i] at out_slots[i].  All-or-nothing: HICR_ERR_DUPLICATE_KEY if a key occurs twice or
+ * (tag, key) exists already in this context, HICR_ERR_INVALID_ARG on a handle that is not one
+ * (or of another tag), HICR_ERR_UNSUPPORTED_SPACE if an owner's memory cannot be mapped from this
+ * device ("Otherwise, it will be rejected"), HICR_ERR_NO_CAPACITY; then no slot is
+ * created.  n == 0 is a valid (empty) exchange.  hicr_slot_unregister drops a global slot again. */
+int hicr_global_exchange(hicr_ctx_t *ctx, uint64_t tag, const hicr_global_handle_t *handles, uint64_t n,
+                         hicr_slot_t *out_slots);
+
+/* The global slot (tag, key) of this context; HICR_ERR_INVALID_SLOT if there is none. */
+int hicr_global_lookup(hicr_ctx_t *ctx, uint64_t tag, uint64_t key, hicr_slot_t *out);
+
+/* Global fence, local half 1: hicr_fence (blocks; returns its deferred error, and still reports),
+ * then one line per global slot of this context into out[0 .. *n) (host pointers; cap = room in
+ * `out`; HICR_ERR_NO_CAPACITY with *n = the number needed if cap is short). */
+int hicr_global_fence_begin(hicr_ctx_t *ctx, hicr_global_count_t *out, uint64_t cap, uint64_t *n);
+
+/* Global fence, local half 2: `all` = the lines of ALL instances (any order).  For every global
+ * slot this context owns, the expected totals are the sums of its lines; blocks until the
+ * owner-side counters on this device have reached them, i.e. until every transfer any instance
+ * had initiated on this context's slots when it entered its fence is complete and visible here:
+ * "suspend execution until the expected number of incoming and outgoing data transfers have been
+ * completed".  HICR_ERR_TIMEOUT after timeout_ms (0 = wait for ever). */
+int hicr_global_fence_end(hicr_ctx_t *ctx, const hicr_global_count_t *all, uint64_t n_all, uint32_t timeout_ms);
+
+/* Owner-side totals of a slot of this context (a local slot that was volunteered, or this
+ * context's own global id of it): messages of ALL instances that named the global slot as source
+ * (sent) / destination (recv).  Defined after hicr_global_fence_end.  Zero for a slot never
+ * volunteered; HICR_ERR_INVALID_ARG for a global slot another instance owns. */
+int hicr_global_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64_t *recv);
 
 /* ---- channels -------------------------------------------------- */
 

@@ -570,8 +570,8 @@ int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, h
         pr.id_src = (uint32_t)si;
         pr.id_dst = (uint32_t)di;
         pr.pad = 0;
-        rc = pipe_run(ctx, &pr, reinterpret_cast<PipeRing *>(ch->d_tab + n_batches * 8), 1, ch->T, ch->C, total, d_batches, 0,
-                      ctx->d_call, &piped);
+        rc = pipe_run(ctx, &pr, reinterpret_cast<PipeRing *>(ch->d_tab + n_batches * 8), 1, ch->T, ch->C, total, d_batches, n_batches,
+                      0, ctx->d_call, &piped);
         if (rc != HICR_OK) return rc;
     }
     if (!piped) {
@@ -702,7 +702,7 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_
             pr[p].id_dst = ids[2 * P + p];
             pr[p].pad = 0;
         }
-        int rc = pipe_run(ctx, pr.data(), m->d_pipe, P, m->T, m->C, N, nullptr, max_batch, nullptr, &piped);
+        int rc = pipe_run(ctx, pr.data(), m->d_pipe, P, m->T, m->C, N, nullptr, 0, max_batch, nullptr, &piped);
         if (rc != HICR_OK) return rc;
     }
     if (!piped) {

@@ -240,6 +240,11 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
     for (int i = 0; i < 2; i++) INIT_CUDA(cudaEventCreate(&ctx->ev[i]));
     INIT_CUDA(cudaDeviceSynchronize());
 #undef INIT_CUDA
+    if (global_setup(ctx) != HICR_OK) {
+        fprintf(stderr, "hicr_init: %s\n", ctx->cuda_error.c_str());
+        hicr_finalize(ctx);
+        return HICR_ERR_CUDA;
+    }
     {
         int rc = engine_setup(ctx);
         if (rc != HICR_OK) {
@@ -260,6 +265,7 @@ int hicr_finalize(hicr_ctx_t *ctx)
     (void)cudaStreamSynchronize(ctx->stream);
     stage_pool_destroy(ctx->stage_pool);
     stage_done_free(ctx->stage_done);
+    global_teardown(ctx);
     cudaFree(ctx->d_slots);
     cudaFree(ctx->d_cnt);
     cudaFree(ctx->d_ctl);
@@ -305,6 +311,10 @@ int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot)
     const int64_t i = slot_find(ctx, slot);
     if (i < 0) return HICR_ERR_INVALID_SLOT;
     if (ctx->ring_refs[i]) return HICR_ERR_BUSY;
+    if (ctx->rows[i].meta & kRowGlobal) {
+        int rc = global_forget(ctx, (uint32_t)i);   // unmap the owner's storage, unpin the local slot behind it
+        if (rc != HICR_OK) return rc;
+    }
     const SlotRow row{0, kInvalidMeta};
     HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + i, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
     ctx->registered_bytes -= row_size(ctx->rows[i]);

@@ -116,6 +116,11 @@ struct EngineArgs {
     uint32_t flag;                   // rec_flag(sequence number of this batch)
     uint32_t skip_barrier;           // the host validated the table and it holds no large descriptor
     uint32_t hand_out;               // kHandOutVote (device tables), or what the host's own count says
+    // Global Memory Slots: per table row of kind GLOBAL the address of the owner's
+    // counters (peer-mapped when the owner is another instance), and this batch's counts per such row
+    const uint64_t *gptr;
+    SlotCnt *gdelta;
+    uint32_t any_global;
 };
 constexpr uint32_t kHandOutVote = 0, kHandOutDynamic = 1, kHandOutStatic = 2;
 
@@ -394,7 +399,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         if (use_hist) {
             for (uint32_t s = tid; s < 2 * n_slots; s += kThreads) {
                 const unsigned v = hist[s];
-                if (v) atomicAdd(s < n_slots ? &a.cnt[s].sent : &a.cnt[s - n_slots].recv, (unsigned long long)v);
+                if (!v) continue;
+                const uint32_t row = s < n_slots ? s : s - n_slots;
+                atomicAdd(s < n_slots ? &a.cnt[row].sent : &a.cnt[row].recv, (unsigned long long)v);
+                // a message on a global slot also counts at the slot's owner (published by the last CTA)
+                if (a.any_global && (slot_row(cache, a.slots, n_slots, row).meta & kRowGlobal))
+                    atomicAdd(s < n_slots ? &a.gdelta[row].sent : &a.gdelta[row].recv, (unsigned long long)v);
             }
         } else {
             // slot table too large for the shared-memory histogram: count straight into the
@@ -408,9 +418,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
                     ss = lo.y & kSlotIndexMask;
                 }
                 const unsigned ms = __match_any_sync(0xffffffffu, ss);
-                if (i < a.n && lane == __ffs(ms) - 1) atomicAdd(&a.cnt[ss].sent, (unsigned long long)__popc(ms));
+                if (i < a.n && lane == __ffs(ms) - 1) {
+                    atomicAdd(&a.cnt[ss].sent, (unsigned long long)__popc(ms));
+                    if (a.any_global && (slot_row(cache, a.slots, n_slots, ss).meta & kRowGlobal))
+                        atomicAdd(&a.gdelta[ss].sent, (unsigned long long)__popc(ms));
+                }
                 const unsigned md = __match_any_sync(0xffffffffu, ds);
-                if (i < a.n && lane == __ffs(md) - 1) atomicAdd(&a.cnt[ds].recv, (unsigned long long)__popc(md));
+                if (i < a.n && lane == __ffs(md) - 1) {
+                    atomicAdd(&a.cnt[ds].recv, (unsigned long long)__popc(md));
+                    if (a.any_global && (slot_row(cache, a.slots, n_slots, ds).meta & kRowGlobal))
+                        atomicAdd(&a.gdelta[ds].recv, (unsigned long long)__popc(md));
+                }
             }
         }
 
@@ -550,6 +568,24 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     if (!sh_flag) return;
     // last CTA: every CTA's copies and counter updates are complete and visible on the device
     // (release increments above, acquired by this CTA's thread 0 and handed on by the barrier).
+    // Global Memory Slots: what this batch moved from / into a global slot is complete, so it now counts
+    // at the slot's owner -- data first (system scope: the owner may be another GPU), then the owner's
+    // counters, which is what lets the owner's fence wait for "the expected number of incoming and
+    // outgoing data transfers" without a message from this instance.
+    if (a.any_global) {
+        for (uint32_t s = tid; s < n_slots; s += kThreads) {
+            const uint64_t g = __ldcg(a.gptr + s);
+            if (!g) continue;
+            const unsigned long long sv = __ldcg(&a.gdelta[s].sent), rv = __ldcg(&a.gdelta[s].recv);
+            if (!(sv | rv)) continue;
+            __threadfence_system();
+            SlotCnt *owner = reinterpret_cast<SlotCnt *>(g);
+            if (sv) atomicAdd_system(&owner->sent, sv);
+            if (rv) atomicAdd_system(&owner->recv, rv);
+            a.gdelta[s].sent = 0;
+            a.gdelta[s].recv = 0;
+        }
+    }
     // Publish the cumulative counters and the completion record as flagged 8-byte words.
     for (uint32_t s = tid; s < a.n_push; s += kThreads) {
         const unsigned long long sv = __ldcg(&a.cnt[s].sent), rv = __ldcg(&a.cnt[s].recv);
@@ -715,6 +751,9 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     a.flag = rec_flag(ctx->batch_seq + 1);
     a.skip_barrier = skip_barrier ? 1u : 0u;
     a.hand_out = hand_out;
+    a.gptr = ctx->d_gptr;
+    a.gdelta = ctx->d_gdelta;
+    a.any_global = ctx->n_global ? 1u : 0u;
 
     // grid: every co-resident CTA unless the host knows the batch is smaller than that
     uint64_t want = std::max<uint64_t>((n + kThreads - 1) / kThreads, units == ~0ull ? (uint64_t)ctx->engine_grid : units);

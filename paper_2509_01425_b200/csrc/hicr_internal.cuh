@@ -537,6 +537,7 @@ struct StageBlock {
 };
 
 class StagePool;
+struct GlobalTable;   // hicr_global.cu: the context's Global Memory Slots, by table index and by (tag, key)
 
 }  // namespace hicr
 
@@ -595,6 +596,17 @@ struct hicr_ctx {
     hicr::CallResult *d_call = nullptr;      // device alias of h_call
     uint64_t call_seq = 0;                   // sequence number of the last host-call push / pop
 
+    // Global Memory Slots (hicr_global.cu).  d_gcnt: owner-side totals of this context's
+    // own slots -- every instance that names a global slot adds to them through d_gptr, which holds, per
+    // table row of kind GLOBAL, the (possibly peer-mapped) address of the owner's d_gcnt entry.  d_gdelta:
+    // what the running batch counted per global row, published to the owner by the batch's last CTA.
+    uint32_t instance = 0, n_instances = 1;
+    hicr::SlotCnt *d_gcnt = nullptr;         // [HICR_MAX_SLOTS]
+    uint64_t *d_gptr = nullptr;              // [HICR_MAX_SLOTS] 0 = not a global row
+    hicr::SlotCnt *d_gdelta = nullptr;       // [HICR_MAX_SLOTS] all-zero between batches
+    uint32_t n_global = 0;                   // live rows of kind GLOBAL
+    hicr::GlobalTable *globals = nullptr;
+
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
     uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
@@ -616,8 +628,11 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
                 int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
 int bad_to_status(unsigned id);
 int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hicr_slot_t *out);
+int global_setup(hicr_ctx *ctx);
+void global_teardown(hicr_ctx *ctx);
+int global_forget(hicr_ctx *ctx, uint32_t index);
 int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t P, uint64_t T, uint64_t C, uint64_t tokens,
-             const uint64_t *d_batches, uint64_t max_batch, CallResult *res, bool *ran);
+             const uint64_t *d_batches, uint64_t n_batches, uint64_t max_batch, CallResult *res, bool *ran);
 StagePool *stage_pool_create(int helpers);
 void stage_pool_destroy(StagePool *p);
 void stage_done_free(std::atomic<uint64_t> *p);
