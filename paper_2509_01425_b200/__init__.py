@@ -11,12 +11,16 @@ from .binding import (  # noqa: F401
     EXPORTS,
     HICR_ERR_BUSY,
     HICR_ERR_CUDA,
+    HICR_ERR_DUPLICATE_KEY,
     HICR_ERR_ILLEGAL_DIRECTION,
     HICR_ERR_INVALID_ARG,
     HICR_ERR_INVALID_SLOT,
     HICR_ERR_NO_CAPACITY,
     HICR_ERR_OUT_OF_BOUNDS,
+    HICR_ERR_TIMEOUT,
     HICR_ERR_UNSUPPORTED_SPACE,
+    HICR_GLOBAL_HANDLE_BYTES,
+    GLOBAL_COUNT_DTYPE,
     HICR_MAX_SLOTS,
     HICR_OK,
     LIB_PATH,
@@ -26,3 +30,4 @@ from .binding import (  # noqa: F401
     Mpsc,
     lib,
 )
+from . import collective  # noqa: F401,E402

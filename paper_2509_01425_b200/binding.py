@@ -27,7 +27,14 @@ HICR_ERR_NO_CAPACITY = -5
 HICR_ERR_CUDA = -6
 HICR_ERR_BUSY = -7
 HICR_ERR_ILLEGAL_DIRECTION = -8
+HICR_ERR_DUPLICATE_KEY = -9
+HICR_ERR_TIMEOUT = -10
 HICR_MAX_SLOTS = 4096
+HICR_GLOBAL_HANDLE_BYTES = 256
+
+# hicr_global_count_t: one line of a global fence's count exchange
+GLOBAL_COUNT_DTYPE = np.dtype([("tag", "<u8"), ("key", "<u8"), ("sent", "<u8"), ("recv", "<u8")])
+assert GLOBAL_COUNT_DTYPE.itemsize == 32
 
 # hicr_desc_t: dst_slot, src_slot, dst_off, src_off, size (PAPER.md:532 argument order)
 DESC_DTYPE = np.dtype(
@@ -43,6 +50,8 @@ EXPORTS = (
     "hicr_channel_push", "hicr_channel_pop", "hicr_channel_stream",
     "hicr_mpsc_create", "hicr_mpsc_destroy", "hicr_mpsc_counters", "hicr_mpsc_stream",
     "hicr_mpsc_locking_stream",
+    "hicr_instance_set", "hicr_global_volunteer", "hicr_global_exchange", "hicr_global_lookup",
+    "hicr_global_fence_begin", "hicr_global_fence_end", "hicr_global_counters",
     "hicr_launch_count", "hicr_profile_enable", "hicr_profile_read",
 )
 
@@ -79,6 +88,13 @@ def _load() -> ctypes.CDLL:
         "hicr_mpsc_counters": (i32, [vp, u32, P(u64), P(u64)]),
         "hicr_mpsc_stream": (i32, [vp, vp, vp, vp, vp, u64, u64]),
         "hicr_mpsc_locking_stream": (i32, [vp, u32, vp, u32, u64, u64, u64]),
+        "hicr_instance_set": (i32, [vp, u32, u32]),
+        "hicr_global_volunteer": (i32, [vp, u64, u64, u32, vp]),
+        "hicr_global_exchange": (i32, [vp, u64, vp, u64, vp]),
+        "hicr_global_lookup": (i32, [vp, u64, u64, P(u32)]),
+        "hicr_global_fence_begin": (i32, [vp, vp, u64, P(u64)]),
+        "hicr_global_fence_end": (i32, [vp, vp, u64, u32]),
+        "hicr_global_counters": (i32, [vp, u32, P(u64), P(u64)]),
         "hicr_launch_count": (i32, [vp, P(u64)]),
         "hicr_profile_enable": (i32, [vp, i32]),
         "hicr_profile_read": (i32, [vp, P(ctypes.c_float)]),
@@ -222,6 +238,74 @@ class Context:
             b, i = ctypes.c_uint64(), ctypes.c_uint64()
             lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
             self._fail(rc, "hicr_fence_expected", first_bad=i.value, batch_index=b.value)
+
+    # ---- Global Memory Slots (the local halves; collective.py carries the bytes between instances)
+    def instance_set(self, instance: int, n_instances: int):
+        rc = lib.hicr_instance_set(self._h, instance, n_instances)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_instance_set")
+
+    def global_volunteer(self, tag: int, key: int, local_slot: int) -> bytes:
+        """hicr_global_volunteer: the 256-byte handle of ``local_slot`` as (tag, key)."""
+        buf = ctypes.create_string_buffer(HICR_GLOBAL_HANDLE_BYTES)
+        rc = lib.hicr_global_volunteer(self._h, tag, key, local_slot, buf)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_global_volunteer")
+        return buf.raw
+
+    def global_exchange(self, tag: int, handles) -> list:
+        """hicr_global_exchange: ``handles`` = the handles of all instances in the agreed order;
+        returns this context's Global Memory Slot id of each."""
+        handles = list(handles)
+        n = len(handles)
+        if any(len(h) != HICR_GLOBAL_HANDLE_BYTES for h in handles):
+            raise ValueError("a global handle is %d bytes" % HICR_GLOBAL_HANDLE_BYTES)
+        blob = ctypes.create_string_buffer(b"".join(handles), max(1, n * HICR_GLOBAL_HANDLE_BYTES))
+        out = (ctypes.c_uint32 * max(1, n))()
+        rc = lib.hicr_global_exchange(self._h, tag, blob, n, out)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_global_exchange")
+        ids = [int(out[i]) for i in range(n)]
+        for g in ids:
+            self._keep[g] = None
+        return ids
+
+    def global_lookup(self, tag: int, key: int) -> int:
+        out = ctypes.c_uint32()
+        rc = lib.hicr_global_lookup(self._h, tag, key, ctypes.byref(out))
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_global_lookup")
+        return out.value
+
+    def global_fence_begin(self) -> np.ndarray:
+        """hicr_global_fence_begin: the blocking local fence, then this context's lines of the
+        count exchange (GLOBAL_COUNT_DTYPE)."""
+        cap = 64
+        while True:
+            out = np.zeros(cap, dtype=GLOBAL_COUNT_DTYPE)
+            n = ctypes.c_uint64()
+            rc = lib.hicr_global_fence_begin(self._h, ctypes.c_void_p(out.ctypes.data), cap, ctypes.byref(n))
+            if rc == HICR_ERR_NO_CAPACITY and n.value > cap:
+                cap = int(n.value)
+                continue
+            if rc != HICR_OK:
+                b, i = ctypes.c_uint64(), ctypes.c_uint64()
+                lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
+                self._fail(rc, "hicr_global_fence_begin", first_bad=i.value, batch_index=b.value)
+            return out[: n.value].copy()
+
+    def global_fence_end(self, all_counts: np.ndarray, timeout_ms: int = 0):
+        a = np.ascontiguousarray(all_counts, dtype=GLOBAL_COUNT_DTYPE)
+        rc = lib.hicr_global_fence_end(self._h, ctypes.c_void_p(a.ctypes.data if a.size else 0), a.size, timeout_ms)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_global_fence_end")
+
+    def global_counters(self, slot: int):
+        s, r = ctypes.c_uint64(), ctypes.c_uint64()
+        rc = lib.hicr_global_counters(self._h, slot, ctypes.byref(s), ctypes.byref(r))
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_global_counters")
+        return s.value, r.value
 
     # ---- channels
     def channel_create(self, ring: int, token_bytes: int, capacity: int) -> "Channel":

@@ -1,0 +1,273 @@
+"""Parity of the Global Memory Slots on the CUDA path
+against the oracle's World: the exchange (counts, lookup, duplicate keys), the three legal
+directions and the rejected fourth, puts and gets between instances, every instance's memory
+image, every slot's counters and the owner-side totals after the global fence -- bit-exact.
+
+Instances are contexts.  Two set-ups: several contexts of this process on cuda:0 (the owner's
+addresses are used as they are), and two PROCESSES on cuda:0 whose storage reaches each other
+through CUDA IPC handles carried by a gloo group -- the path a one-process-per-GPU job takes over
+NVLink.  (The pod has one GPU: the two processes' kernels never wait for each other -- each
+fences locally, the count exchange runs on the host.)"""
+import json
+import os
+import subprocess
+import sys
+
+import numpy as np
+import pytest
+
+import oracle
+import workloads as W
+from global_common import NAMES, descs_for, oracle_run
+from oracle.world import World
+
+pytestmark = pytest.mark.gpu
+
+torch = pytest.importorskip("torch")
+
+STATUS = {"ok": oracle.OK, "illegal_direction": oracle.ERR_ILLEGAL_DIRECTION, "duplicate_key": oracle.ERR_DUPLICATE_KEY,
+          "out_of_bounds": oracle.ERR_OUT_OF_BOUNDS}
+
+
+@pytest.fixture(scope="module")
+def hicr():
+    if not torch.cuda.is_available():
+        pytest.fail("GPU tests need a CUDA device (there is no CPU fallback)")
+    import paper_2509_01425_b200 as h
+    return h
+
+
+def _instances(hicr, n):
+    ctxs = [hicr.Context(0, torch.cuda.current_stream().cuda_stream) for _ in range(n)]
+    for i, c in enumerate(ctxs):
+        c.instance_set(i, n)
+    return ctxs
+
+
+def _close(ctxs):
+    for c in ctxs:
+        c.close()
+
+
+def _bytes(s):
+    return np.frombuffer(s.encode("ascii"), dtype=np.uint8).copy()
+
+
+def _one(dst, dst_off, src, src_off, size):
+    return W.make_descs([dst], [src], [dst_off], [src_off], [size])
+
+
+def test_status_codes_match_the_oracle(hicr):
+    assert hicr.HICR_ERR_ILLEGAL_DIRECTION == oracle.ERR_ILLEGAL_DIRECTION
+    assert hicr.HICR_ERR_DUPLICATE_KEY == oracle.ERR_DUPLICATE_KEY
+
+
+@pytest.mark.parametrize("device_table", [False, True])
+def test_golden_directions_on_gpu(hicr, golden_dir, device_table):
+    """The four slot-kind pairs: same verdict, same first bad
+    index, same bytes and counters as the oracle, host- and device-validated."""
+    cases = json.load(open(os.path.join(golden_dir, "global_examples.json")))["directions"]
+    for c in cases:
+        world = World(2)
+        mem = [[np.full(32, 1 + 2 * i, np.uint8), np.full(32, 2 + 2 * i, np.uint8)] for i in range(2)]
+        oid = [[world.inst[i].slot_register(a) for a in mem[i]] for i in range(2)]
+        rc, og = world.exchange(7, [[(0, oid[0][1])], [(1, oid[1][1])]])
+        assert rc == oracle.OK
+        ctxs = _instances(hicr, 2)
+        try:
+            bufs = [[torch.from_numpy(a.copy()).cuda() for a in mem[i]] for i in range(2)]
+            gid = [[ctxs[i].slot_register(t) for t in bufs[i]] for i in range(2)]
+            assert gid == oid
+            gg = hicr.collective.exchange_in_process(ctxs, 7, [[(0, gid[0][1])], [(1, gid[1][1])]])
+            assert gg == og
+            slot = {"L": gid[0][0], "G": gg[0][1]}
+            dst, src = slot[c["dst"]], slot[c["src"]]
+            if c["dst"] == c["src"] == "G":
+                src = gg[0][0]
+            if c["dst"] == c["src"] == "L":
+                src = gid[0][1]
+            d = np.concatenate([_one(gid[0][0], 0, gid[0][1], 0, 4), _one(dst, 4, src, 8, 16)])   # a valid one first
+            orc, obad = world.inst[0].memcpy_batch(d)
+            assert orc == STATUS[c["status"]], c["cite"]
+            if device_table:
+                t = torch.from_numpy(d.view(np.uint8).copy()).cuda()
+                ctxs[0].memcpy_batch(t, n=len(d))
+                if orc == oracle.OK:
+                    ctxs[0].fence()
+                else:
+                    with pytest.raises(hicr.HicrError) as e:
+                        ctxs[0].fence()
+                    assert (e.value.status, e.value.first_bad) == (orc, obad), c["cite"]
+            elif orc == oracle.OK:
+                ctxs[0].memcpy_batch(d)
+            else:
+                with pytest.raises(hicr.HicrError) as e:
+                    ctxs[0].memcpy_batch(d)
+                assert (e.value.status, e.value.first_bad) == (orc, obad), c["cite"]
+            world.fence_all()
+            hicr.collective.fence_in_process(ctxs)
+            for i in range(2):
+                for a, t in zip(mem[i], bufs[i]):
+                    assert t.cpu().numpy().tobytes() == a.tobytes(), c["cite"]          # rejected = no effect
+                for s in list(gid[i]) + list(gg[i].values()):
+                    assert ctxs[i].slot_counters(s) == world.inst[i].slot_counters(s), c["cite"]
+                assert ctxs[i].global_counters(gid[i][1]) == world.inst[i].slot_global_counters(oid[i][1]), c["cite"]
+        finally:
+            _close(ctxs)
+
+
+def test_golden_exchange_counts_lookup_and_duplicates(hicr, golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "global_examples.json")))
+    for c in g["exchange"]:
+        n = c["contributions"]
+        ctxs = _instances(hicr, len(n))
+        try:
+            keep, contrib, key = [], [], 0
+            for i, k in enumerate(n):
+                mine = []
+                for _ in range(k):
+                    t = torch.zeros(8 + key, dtype=torch.uint8, device="cuda")
+                    keep.append(t)
+                    mine.append((key, ctxs[i].slot_register(t)))
+                    key += 1
+                contrib.append(mine)
+            out = hicr.collective.exchange_in_process(ctxs, 7, contrib)
+            for i in range(len(n)):
+                assert len(out[i]) == c["received_by_each"] == sum(n), c["cite"]
+                for k in range(sum(n)):
+                    assert ctxs[i].global_lookup(7, k) == out[i][k]
+                for bad in ((7, 99), (8, 0)):                                            # unknown key / unknown tag
+                    with pytest.raises(hicr.HicrError) as e:
+                        ctxs[i].global_lookup(*bad)
+                    assert e.value.status == hicr.HICR_ERR_INVALID_SLOT
+        finally:
+            _close(ctxs)
+    # duplicate keys: all-or-nothing, on every instance
+    ctxs = _instances(hicr, 2)
+    try:
+        a, b = (torch.zeros(8, dtype=torch.uint8, device="cuda") for _ in range(2))
+        sa, sb = ctxs[0].slot_register(a), ctxs[1].slot_register(b)
+        with pytest.raises(hicr.HicrError) as e:
+            hicr.collective.exchange_in_process(ctxs, 7, [[(0, sa)], [(0, sb)]])
+        assert e.value.status == STATUS[g["duplicate_key"]["status"]], g["duplicate_key"]["cite"]
+        with pytest.raises(hicr.HicrError):
+            ctxs[0].global_lookup(7, 0)                                                  # nothing was created
+        out = hicr.collective.exchange_in_process(ctxs, 7, [[(0, sa)], [(1, sb)]])
+        hicr.collective.exchange_in_process(ctxs, 8, [[(0, sa)], [(1, sb)]])             # same keys, another tag
+        with pytest.raises(hicr.HicrError) as e:
+            hicr.collective.exchange_in_process(ctxs, 7, [[(1, sa)], []])                # (7, 1) exists
+        assert e.value.status == hicr.HICR_ERR_DUPLICATE_KEY
+        # only local slots are volunteered; a local slot behind a global one cannot be unregistered
+        with pytest.raises(hicr.HicrError) as e:
+            ctxs[0].global_volunteer(9, 5, out[0][1])
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        with pytest.raises(hicr.HicrError) as e:
+            ctxs[0].slot_unregister(sa)
+        assert e.value.status == hicr.HICR_ERR_BUSY
+        ctxs[0].slot_unregister(out[0][0])
+        ctxs[0].slot_unregister(ctxs[0].global_lookup(8, 0))
+        ctxs[0].slot_unregister(sa)
+        with pytest.raises(hicr.HicrError):
+            ctxs[0].global_lookup(7, 0)
+    finally:
+        _close(ctxs)
+
+
+def test_golden_put_get_self_zero_oob_on_gpu(hicr, golden_dir):
+    g = json.load(open(os.path.join(golden_dir, "global_examples.json")))
+    ctxs = _instances(hicr, 2)
+    try:
+        bufs = [[torch.zeros(32, dtype=torch.uint8, device="cuda") for _ in range(2)] for _ in range(2)]
+        ids = [[ctxs[i].slot_register(t) for t in bufs[i]] for i in range(2)]
+        gg = hicr.collective.exchange_in_process(ctxs, 7, [[(0, ids[0][1])], [(1, ids[1][1])]])
+        put = _bytes(g["put"]["payload"])
+        bufs[0][0][:16] = torch.from_numpy(put).cuda()
+        ctxs[0].memcpy_batch(_one(gg[0][1], 8, ids[0][0], 0, 16))
+        hicr.collective.fence_in_process(ctxs)
+        assert bufs[1][1][8:24].cpu().numpy().tobytes() == put.tobytes(), g["put"]["cite"]
+        assert int(bufs[1][1][:8].sum()) == 0 and int(bufs[1][1][24:].sum()) == 0
+        get = _bytes(g["get"]["payload"])
+        bufs[1][1][:16] = torch.from_numpy(get).cuda()
+        ctxs[0].memcpy_batch(_one(ids[0][0], 16, gg[0][1], 0, 16))
+        hicr.collective.fence_in_process(ctxs)
+        assert bufs[0][0][16:32].cpu().numpy().tobytes() == get.tobytes(), g["get"]["cite"]
+        me = _bytes(g["self_get"]["payload"])
+        bufs[0][1][:16] = torch.from_numpy(me).cuda()
+        ctxs[0].memcpy_batch(_one(ids[0][0], 0, gg[0][0], 0, 16))
+        hicr.collective.fence_in_process(ctxs)
+        assert bufs[0][0][:16].cpu().numpy().tobytes() == me.tobytes(), g["self_get"]["cite"]
+        before = [t.clone() for pair in bufs for t in pair]
+        c0, g0 = ctxs[0].slot_counters(gg[0][1]), ctxs[1].global_counters(ids[1][1])
+        ctxs[0].memcpy_batch(_one(gg[0][1], 32, ids[0][0], 32, 0))
+        hicr.collective.fence_in_process(ctxs)
+        assert all(torch.equal(a, b) for a, b in zip(before, [t for pair in bufs for t in pair])), g["zero_put"]["cite"]
+        assert ctxs[0].slot_counters(gg[0][1]) == (c0[0], c0[1] + 1), g["zero_put"]["cite"]
+        assert ctxs[1].global_counters(ids[1][1]) == (g0[0], g0[1] + 1), g["zero_put"]["cite"]
+        with pytest.raises(hicr.HicrError) as e:
+            ctxs[0].memcpy_batch(_one(ids[0][0], 0, gg[0][1], 20, 16))
+        assert (e.value.status, e.value.first_bad) == (STATUS[g["oob_get"]["status"]], 0), g["oob_get"]["cite"]
+    finally:
+        _close(ctxs)
+
+
+def _compare_with_oracle(hicr, w, ctxs, bufs, ids, gg):
+    world, mem, oids, og = oracle_run(w)
+    assert ids == oids and gg == og
+    for i in range(w.n_instances):
+        for k in NAMES:
+            assert bufs[i][k].cpu().numpy().tobytes() == mem[i][k].tobytes(), "instance %d %s" % (i, k)
+        for s in list(ids[i].values()) + list(gg[i].values()):
+            assert ctxs[i].slot_counters(s) == world.inst[i].slot_counters(s), "instance %d slot %d" % (i, s)
+        for k in NAMES:
+            assert ctxs[i].global_counters(ids[i][k]) == world.inst[i].slot_global_counters(oids[i][k]), (i, k)
+
+
+@pytest.mark.parametrize("n_inst,device_tables,big", [(2, False, False), (3, True, False), (4, True, True), (2, False, True)])
+def test_copy_graph_between_instances(hicr, n_inst, device_tables, big):
+    """Random Local-to-Local / put / get transfers dealt to n instances, one global fence: every
+    instance's four buffers, all per-slot counters and the owners' totals equal the oracle's.
+    `big`: sizes up to 300 KB, so the chunk queue and the TMA path carry global slots too."""
+    w = (W.global_copy_graph(n_inst, per_buffer=24, src_bytes=1 << 20, dst_bytes=8 << 20, max_size=300000, seed=W.BASE_SEED + 5)
+         if big else W.global_copy_graph(n_inst))
+    ctxs = _instances(hicr, n_inst)
+    try:
+        bufs = [{k: torch.from_numpy(w.image(i, k)).cuda() for k in NAMES} for i in range(n_inst)]
+        ids = [{k: ctxs[i].slot_register(bufs[i][k]) for k in NAMES} for i in range(n_inst)]
+        gg = hicr.collective.exchange_in_process(
+            ctxs, w.tag, [[(2 * i, ids[i]["gsrc"]), (2 * i + 1, ids[i]["gdst"])] for i in range(n_inst)])
+        keep = []
+        for i in range(n_inst):
+            d = descs_for(w, i, ids[i], gg[i])
+            if device_tables:
+                keep.append(torch.from_numpy(d.view(np.uint8).copy()).cuda())
+                ctxs[i].memcpy_batch(keep[-1], n=len(d))
+            else:
+                ctxs[i].memcpy_batch(d)
+        hicr.collective.fence_in_process(ctxs)
+        _compare_with_oracle(hicr, w, ctxs, bufs, ids, gg)
+    finally:
+        _close(ctxs)
+
+
+@pytest.mark.timeout(600)
+def test_two_processes_over_cuda_ipc():
+    """Two processes, one context each, on cuda:0; handles and fence counts travel over a gloo
+    group; the storage of the other process is reached through CUDA IPC.  Each rank compares its
+    own memory, counters and owner-side totals with the oracle's World (tests/global_two_proc.py
+    exits non-zero on any difference)."""
+    here = os.path.dirname(os.path.abspath(__file__))
+    port = 29500 + os.getpid() % 2000
+    env = dict(os.environ, MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), WORLD_SIZE="2")
+    procs = [subprocess.Popen([sys.executable, os.path.join(here, "global_two_proc.py")], env=dict(env, RANK=str(r)),
+                              stdout=subprocess.PIPE, stderr=subprocess.STDOUT) for r in range(2)]
+    outs = []
+    for p in procs:
+        try:
+            out, _ = p.communicate(timeout=500)
+        except subprocess.TimeoutExpired:
+            p.kill()
+            out, _ = p.communicate()
+        outs.append(out.decode(errors="replace"))
+    for r, (p, out) in enumerate(zip(procs, outs)):
+        assert p.returncode == 0, "rank %d:\n%s" % (r, out[-3000:])
+        assert "global two-process parity ok" in out

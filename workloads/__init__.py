@@ -2,4 +2,4 @@
 
 Holds none of the method's arithmetic (see generators.py)."""
 from .generators import *  # noqa: F401,F403
-from .generators import BASE_SEED, DESC_DTYPE, CopyWorkload, ChannelWorkload  # noqa: F401
+from .generators import BASE_SEED, DESC_DTYPE, CopyWorkload, ChannelWorkload, GlobalWorkload  # noqa: F401

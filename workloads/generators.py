@@ -301,3 +301,56 @@ def tagged_sources(producers: int, n_tokens: int, token_bytes: int, seed: int = 
         a[:, :8] = tag.view(np.uint8).reshape(n_tokens, 8)
         out.append(np.ascontiguousarray(a.reshape(-1)))
     return out
+
+
+# ---------------------------------------------------------------------------------- global slots
+@dataclass
+class GlobalWorkload:
+    """A copy graph over several instances ("randomized
+    copy-graph").  Every instance has four buffers: ``lsrc`` / ``ldst`` stay local, ``gsrc`` /
+    ``gdst`` are volunteered under ``tag`` with keys 2 i and 2 i + 1.  ``plans[i]`` lists the
+    transfers instance i initiates as (dst, dst_off, src, src_off, size) with dst / src =
+    ("L", name) for one of its own local buffers or ("G", key) for a global slot.  Sources are
+    only read and destinations only written, destination ranges are pairwise disjoint over ALL
+    instances (the epoch precondition of reading 5, extended to the global epoch), and no
+    transfer names two global slots."""
+    n_instances: int
+    tag: int
+    sizes: dict
+    plans: list
+    seed: int
+
+    def image(self, instance: int, name: str) -> np.ndarray:
+        return random_bytes(rng_for(6, 100 * instance + ("lsrc", "ldst", "gsrc", "gdst").index(name), self.seed),
+                            self.sizes[name])
+
+
+def global_copy_graph(n_instances: int = 2, per_buffer: int = 12, src_bytes: int = 4096, dst_bytes: int = 65536,
+                      max_size: int = 3000, seed: int = BASE_SEED, tag: int = 3) -> GlobalWorkload:
+    """Local-to-Local, Local-to-Global (put) and Global-to-Local (get) transfers dealt to random
+    initiators; sizes uniform in 0..max_size (zero-size transfers included), byte-granular offsets,
+    destinations by gaps composition."""
+    rng = rng_for(6, 0, seed + n_instances)
+    plans = [[] for _ in range(n_instances)]
+    for owner in range(n_instances):
+        for kind in ("ldst", "gdst"):
+            sizes = rng.integers(0, max_size + 1, size=per_buffer)
+            offs = gaps_composition(rng, sizes, 0, dst_bytes)
+            for sz, off in zip(sizes, offs):
+                sz, off = int(sz), int(off)
+                if kind == "ldst":
+                    init = owner                                     # a local slot is reachable by its instance only
+                    dst = ("L", "ldst")
+                    src_owner = int(rng.integers(0, n_instances))
+                    src = ("L", "lsrc") if (src_owner == init and rng.random() < 0.5) else ("G", 2 * src_owner)
+                else:
+                    init = int(rng.integers(0, n_instances))         # anyone may put into a global slot
+                    dst = ("G", 2 * owner + 1)
+                    src = ("L", "lsrc")
+                so = int(rng.integers(0, src_bytes - min(sz, src_bytes) + 1))
+                plans[init].append((dst, off, src, so, min(sz, src_bytes)))
+    for p in plans:
+        order = rng.permutation(len(p))
+        p[:] = [p[j] for j in order]
+    sizes = {"lsrc": src_bytes, "ldst": dst_bytes, "gsrc": src_bytes, "gdst": dst_bytes}
+    return GlobalWorkload(n_instances, tag, sizes, plans, seed)
