@@ -162,6 +162,25 @@ int hicr_fence_async(hicr_ctx_t *ctx);
  * by hicr_fence. */
 int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64_t recv);
 
+/* ---- replayable chains ("lets config 4 run as one CUDA graph") ---------------
+ * Between hicr_graph_begin and hicr_graph_end, hicr_memcpy_batch (device-resident tables only) and
+ * hicr_fence_async are RECORDED on the context's stream instead of executed (CUDA stream capture);
+ * hicr_graph_launch then enqueues the whole recorded chain with one call, as often as wanted.
+ * Every replay validates, bins, copies and counts on the device exactly like the calls it
+ * records; completion, counters and deferred errors come with the next blocking hicr_fence,
+ * whose batch_index counts the batches since the last blocking fence as usual.  The tables must
+ * stay alive and the slot table unchanged from hicr_graph_begin to the last launch
+ * (HICR_ERR_INVALID_ARG from hicr_graph_launch otherwise).  While recording, every other call
+ * that would enqueue work on the stream returns HICR_ERR_BUSY.  A chain holds at most 64 batches
+ * (HICR_ERR_NO_CAPACITY); max_descs_per_batch sizes the work queues up front.  The context must
+ * have been created on a stream of its own (HICR_ERR_INVALID_ARG on the legacy default stream,
+ * which CUDA cannot capture). */
+typedef struct hicr_graph hicr_graph_t;
+int hicr_graph_begin(hicr_ctx_t *ctx, uint64_t max_descs_per_batch);
+int hicr_graph_end(hicr_ctx_t *ctx, hicr_graph_t **out);
+int hicr_graph_launch(hicr_graph_t *g);
+int hicr_graph_destroy(hicr_graph_t *g);
+
 /* After hicr_fence returned a deferred error: which batch of that epoch (0-based) and
  * which descriptor index in it was the first bad one.  Host pointers out (may be NULL). */
 int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad);

@@ -52,6 +52,7 @@ EXPORTS = (
     "hicr_mpsc_locking_stream",
     "hicr_instance_set", "hicr_global_volunteer", "hicr_global_exchange", "hicr_global_lookup",
     "hicr_global_fence_begin", "hicr_global_fence_end", "hicr_global_counters",
+    "hicr_graph_begin", "hicr_graph_end", "hicr_graph_launch", "hicr_graph_destroy",
     "hicr_launch_count", "hicr_profile_enable", "hicr_profile_read",
 )
 
@@ -95,6 +96,10 @@ def _load() -> ctypes.CDLL:
         "hicr_global_fence_begin": (i32, [vp, vp, u64, P(u64)]),
         "hicr_global_fence_end": (i32, [vp, vp, u64, u32]),
         "hicr_global_counters": (i32, [vp, u32, P(u64), P(u64)]),
+        "hicr_graph_begin": (i32, [vp, u64]),
+        "hicr_graph_end": (i32, [vp, P(vp)]),
+        "hicr_graph_launch": (i32, [vp]),
+        "hicr_graph_destroy": (i32, [vp]),
         "hicr_launch_count": (i32, [vp, P(u64)]),
         "hicr_profile_enable": (i32, [vp, i32]),
         "hicr_profile_read": (i32, [vp, P(ctypes.c_float)]),
@@ -239,6 +244,21 @@ class Context:
             lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
             self._fail(rc, "hicr_fence_expected", first_bad=i.value, batch_index=b.value)
 
+    # ---- replayable chains (hicr_graph_*)
+    def graph_begin(self, max_descs_per_batch: int):
+        rc = lib.hicr_graph_begin(self._h, max_descs_per_batch)
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_graph_begin")
+
+    def graph_end(self) -> "Graph":
+        h = ctypes.c_void_p()
+        rc = lib.hicr_graph_end(self._h, ctypes.byref(h))
+        if rc != HICR_OK:
+            self._fail(rc, "hicr_graph_end")
+        g = Graph(self, h)
+        self._children.append(g)
+        return g
+
     # ---- Global Memory Slots (the local halves; collective.py carries the bytes between instances)
     def instance_set(self, instance: int, n_instances: int):
         rc = lib.hicr_instance_set(self._h, instance, n_instances)
@@ -347,6 +367,25 @@ class Context:
         if rc != HICR_OK:
             self._fail(rc, "hicr_profile_read")
         return [float(x) for x in ms]
+
+
+class Graph:
+    """A recorded chain of batches (hicr_graph_*)."""
+
+    def __init__(self, ctx: Context, h):
+        self._ctx, self._h = ctx, h
+
+    def launch(self):
+        rc = lib.hicr_graph_launch(self._h)
+        if rc != HICR_OK:
+            self._ctx._fail(rc, "hicr_graph_launch")
+
+    def close(self):
+        if self._h:
+            lib.hicr_graph_destroy(self._h)
+            self._h = None
+            if self in self._ctx._children:
+                self._ctx._children.remove(self)
 
 
 class Channel:

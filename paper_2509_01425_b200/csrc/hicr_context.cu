@@ -91,7 +91,7 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence)
     for (uint32_t k = 0; k < nb; k++) {
         const uint32_t b = k == 0 ? nb - 1 : k - 1;   // last batch first, then 0 .. nb-2
         const uint64_t seq = ctx->batch_seq - (nb - 1 - b);
-        int rc = wait_words(ctx, ctx->h_rec[b].w, kRwUsed, rec_flag(seq), words);
+        int rc = wait_words(ctx, ctx->h_rec[(seq - 1) % kRecRing].w, kRwUsed, rec_flag(seq), words);
         if (rc != HICR_OK) return rc;
         if (b == nb - 1) {
             ctx->last_t[0] = join64(words[kRwTStartLo], words[kRwTStartHi]);
@@ -140,6 +140,7 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence)
 // zeroed counters; stream-ordered after everything already enqueued.  flags = kRowGlobal / kRowRemote.
 int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hicr_slot_t *out)
 {
+    if (ctx->capturing) return HICR_ERR_BUSY;
     uint32_t i;
     if (!ctx->free_idx.empty()) i = ctx->free_idx.back();
     else if (ctx->rows.size() < HICR_MAX_SLOTS) i = (uint32_t)ctx->rows.size();
@@ -166,6 +167,7 @@ int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hi
     }
     ctx->registered_bytes += size;
     ctx->push_stale = true;
+    ctx->table_version++;
     *out = (hicr_slot_t)((g << kSlotIndexBits) | i);
     return HICR_OK;
 }
@@ -308,6 +310,7 @@ int hicr_slot_register(hicr_ctx_t *ctx, void *dev_ptr, uint64_t size, hicr_slot_
 int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;
     const int64_t i = slot_find(ctx, slot);
     if (i < 0) return HICR_ERR_INVALID_SLOT;
     if (ctx->ring_refs[i]) return HICR_ERR_BUSY;
@@ -320,6 +323,7 @@ int hicr_slot_unregister(hicr_ctx_t *ctx, hicr_slot_t slot)
     ctx->registered_bytes -= row_size(ctx->rows[i]);
     ctx->rows[i] = row;
     ctx->push_stale = true;
+    ctx->table_version++;
     // the index can be handed out again under the next generation (ids kept from before then name
     // nothing); an index that has used up its generations is retired
     if (ctx->gen[i] < kMaxGen) {
@@ -344,6 +348,7 @@ static int close_epoch(hicr_ctx *ctx);
 int hicr_fence(hicr_ctx_t *ctx)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;
     if (!ctx->epoch_open) {
         // nothing outstanding: return at once
         ctx->last_error = HICR_OK;
@@ -379,6 +384,7 @@ int hicr_fence_async(hicr_ctx_t *ctx)
 int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64_t recv)
 {
     if (!ctx) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;
     const int64_t si = slot_find(ctx, slot);
     if (si < 0) return HICR_ERR_INVALID_SLOT;
     SlotCnt &c = ctx->cnt[si];
@@ -391,7 +397,7 @@ int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64
         // flags agree comes from one batch; counters only grow, so the first such snapshot that
         // reaches the expected counts ends the wait.
         const unsigned long long *w = ctx->h_rec[kRecRing].w + (size_t)si * kPushWordsPerSlot;
-        const unsigned long long *last = ctx->h_rec[ctx->batches_in_epoch - 1].w;
+        const unsigned long long *last = ctx->h_rec[(ctx->batch_seq - 1) % kRecRing].w;
         const uint32_t last_flag = rec_flag(ctx->batch_seq);
         const uint64_t lo_seq = std::max(ctx->born[si], ctx->batch_seq - ctx->batches_in_epoch);
         unsigned spins = 0;

@@ -110,10 +110,12 @@ struct EngineArgs {
     WorkItem *chunk_q;
     uint64_t chunk_cap;
     SlotCnt *cnt;                    // [HICR_MAX_SLOTS] cumulative message counters
-    unsigned long long *rec;         // this batch's record words (device alias of mapped pinned memory)
+    HostRecord *rec_ring;            // kRecRing completion records (device alias of mapped pinned memory); batch number
+                                     // seq (1-based, counted on the device in Ctl::seq) writes record (seq - 1) % kRecRing
+                                     // with flag rec_flag(seq): nothing in the arguments names the launch, so a
+                                     // captured launch can be replayed (hicr_graph_*)
     unsigned long long *push;        // [kPushWordsPerSlot * kPushSlots] pushed counter words (mapped pinned memory)
     uint32_t n_push;
-    uint32_t flag;                   // rec_flag(sequence number of this batch)
     uint32_t skip_barrier;           // the host validated the table and it holds no large descriptor
     uint32_t hand_out;               // kHandOutVote (device tables), or what the host's own count says
     // Global Memory Slots: per table row of kind GLOBAL the address of the owner's
@@ -204,6 +206,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     __shared__ unsigned sh_ticket[2];
     __shared__ WorkItem sh_item[2];              // queue items of the current and the next chunk
     __shared__ unsigned sh_flag;
+    __shared__ unsigned long long sh_seq;        // last CTA: this batch's sequence number
     __shared__ unsigned long long sh_sync;       // the barrier word as the last poll saw it
     __shared__ unsigned sh_first1;               // first descriptor of the CTA's second tickets (warp w: + w x cnt1)
     __shared__ unsigned sh_small[2];             // bytes and count of the small descriptors this CTA validated
@@ -563,9 +566,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
 
     // ================================================================ finish (feeds a7)
     __syncthreads();
-    if (tid == 0) sh_flag = atom_inc_acq_rel_u32(&ctl->done) == gridDim.x - 1;
+    if (tid == 0) {
+        sh_flag = atom_inc_acq_rel_u32(&ctl->done) == gridDim.x - 1;
+        if (sh_flag) sh_seq = __ldcg(&ctl->seq) + 1;   // batches of a context run one after the other: one writer
+    }
     __syncthreads();
     if (!sh_flag) return;
+    const unsigned long long seq = sh_seq;
+    const uint32_t flag = rec_flag(seq);
+    unsigned long long *rec = a.rec_ring[(seq - 1) % kRecRing].w;
     // last CTA: every CTA's copies and counter updates are complete and visible on the device
     // (release increments above, acquired by this CTA's thread 0 and handed on by the barrier).
     // Global Memory Slots: what this batch moved from / into a global slot is complete, so it now counts
@@ -590,24 +599,25 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     for (uint32_t s = tid; s < a.n_push; s += kThreads) {
         const unsigned long long sv = __ldcg(&a.cnt[s].sent), rv = __ldcg(&a.cnt[s].recv);
         unsigned long long *w = a.push + (size_t)s * kPushWordsPerSlot;
-        put_word(w + 0, (uint32_t)sv, a.flag);
-        put_word(w + 1, (uint32_t)(sv >> 32), a.flag);
-        put_word(w + 2, (uint32_t)rv, a.flag);
-        put_word(w + 3, (uint32_t)(rv >> 32), a.flag);
+        put_word(w + 0, (uint32_t)sv, flag);
+        put_word(w + 1, (uint32_t)(sv >> 32), flag);
+        put_word(w + 2, (uint32_t)rv, flag);
+        put_word(w + 3, (uint32_t)(rv >> 32), flag);
     }
     if (tid == 0) {
         const unsigned long long bad = __ldcg(&ctl->bad_inv), t0 = __ldcg(&ctl->t_start), t1 = __ldcg(&ctl->t_mid),
                                  t2 = globaltimer();
-        put_word(a.rec + kRwBadLo, (uint32_t)bad, a.flag);
-        put_word(a.rec + kRwBadHi, (uint32_t)(bad >> 32), a.flag);
-        put_word(a.rec + kRwNChunk, (uint32_t)(sync >> kSyncChunkShift), a.flag);
-        put_word(a.rec + kRwTStartLo, (uint32_t)t0, a.flag);
-        put_word(a.rec + kRwTStartHi, (uint32_t)(t0 >> 32), a.flag);
-        put_word(a.rec + kRwTMidLo, (uint32_t)t1, a.flag);
-        put_word(a.rec + kRwTMidHi, (uint32_t)(t1 >> 32), a.flag);
-        put_word(a.rec + kRwTEndLo, (uint32_t)t2, a.flag);
-        put_word(a.rec + kRwTEndHi, (uint32_t)(t2 >> 32), a.flag);
+        put_word(rec + kRwBadLo, (uint32_t)bad, flag);
+        put_word(rec + kRwBadHi, (uint32_t)(bad >> 32), flag);
+        put_word(rec + kRwNChunk, (uint32_t)(sync >> kSyncChunkShift), flag);
+        put_word(rec + kRwTStartLo, (uint32_t)t0, flag);
+        put_word(rec + kRwTStartHi, (uint32_t)(t0 >> 32), flag);
+        put_word(rec + kRwTMidLo, (uint32_t)t1, flag);
+        put_word(rec + kRwTMidHi, (uint32_t)(t1 >> 32), flag);
+        put_word(rec + kRwTEndLo, (uint32_t)t2, flag);
+        put_word(rec + kRwTEndHi, (uint32_t)(t2 >> 32), flag);
         // self-clean: the next batch on the stream finds an all-zero control block
+        ctl->seq = seq;
         ctl->bad_inv = 0;
         ctl->sync = 0;
         ctl->ticket = 0;
@@ -618,12 +628,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
 
 static int ensure_queues(hicr_ctx *ctx, uint64_t n)
 {
+    // (while a chain is being recorded nothing may synchronise the stream: hicr_graph_begin sized the queue)
     // With pairwise-disjoint destinations (the epoch precondition) a batch expands into
     // at most 2 n + registered_bytes / kChunkBytes chunks (a first and a last partial one
     // per descriptor).
     const uint64_t need = 2 * n + ctx->registered_bytes / kChunkBytes + 64;
     if (need > ctx->chunk_cap) {
-        if (need > kMaxChunks) return HICR_ERR_NO_CAPACITY;
+        if (need > kMaxChunks || ctx->capturing) return HICR_ERR_NO_CAPACITY;
         uint64_t cap = std::min(std::max(need, ctx->chunk_cap * 2), kMaxChunks);
         HICR_CUDA(ctx, cudaStreamSynchronize(ctx->stream));
         if (ctx->d_chunk) HICR_CUDA(ctx, cudaFree(ctx->d_chunk));
@@ -692,9 +703,14 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     if (n >= (1ull << 31)) return HICR_ERR_NO_CAPACITY;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
 
+    if (ctx->capturing) {
+        // recorded, not executed: only what the replay can do again -- a device-resident table
+        if (!descs_on_device) return HICR_ERR_INVALID_ARG;
+        if (ctx->captured_batches == kRecRing) return HICR_ERR_NO_CAPACITY;
+    }
     // before anything of this batch is staged: an epoch that has used up its completion records
     // drains them (and recycles the staging blocks of the batches that are then complete)
-    if (ctx->batches_in_epoch == kRecRing) {
+    if (!ctx->capturing && ctx->batches_in_epoch == kRecRing) {
         int rc = drain_epoch(ctx, false);
         if (rc != HICR_OK) return rc;
     }
@@ -745,10 +761,9 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     a.chunk_q = ctx->d_chunk;
     a.chunk_cap = ctx->chunk_cap;
     a.cnt = ctx->d_cnt;
-    a.rec = ctx->d_rec[ctx->batches_in_epoch].w;
+    a.rec_ring = ctx->d_rec;
     a.push = ctx->d_rec[kRecRing].w;
     a.n_push = std::min<uint32_t>(a.n_slots, kPushSlots);
-    a.flag = rec_flag(ctx->batch_seq + 1);
     a.skip_barrier = skip_barrier ? 1u : 0u;
     a.hand_out = hand_out;
     a.gptr = ctx->d_gptr;
@@ -759,6 +774,12 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     uint64_t want = std::max<uint64_t>((n + kThreads - 1) / kThreads, units == ~0ull ? (uint64_t)ctx->engine_grid : units);
     const unsigned grid = (unsigned)std::max<uint64_t>(1, std::min<uint64_t>(want, (uint64_t)ctx->engine_grid));
     void *args[] = {&a};
+    if (ctx->capturing) {
+        HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args,
+                                                   engine_smem_bytes(a.n_slots), ctx->stream));
+        ctx->captured_batches++;
+        return HICR_OK;   // the context's books are kept by hicr_graph_launch
+    }
     if (ctx->profiling) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
     HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args,
                                                engine_smem_bytes(a.n_slots), ctx->stream));
@@ -772,5 +793,83 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     ctx->epoch_open = true;
     ctx->last_n_push = a.n_push;
     ctx->push_stale = false;
+    return HICR_OK;
+}
+
+// ---------------------------------------------------------------- replayable chains (hicr_graph_*)
+struct hicr_graph {
+    hicr_ctx *ctx = nullptr;
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    uint32_t n_batches = 0, n_push = 0;
+    uint64_t table_version = 0;
+};
+
+extern "C" int hicr_graph_begin(hicr_ctx_t *ctx, uint64_t max_descs_per_batch)
+{
+    if (!ctx || max_descs_per_batch >= (1ull << 31)) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;
+    if (!ctx->stream) return HICR_ERR_INVALID_ARG;   // the legacy default stream cannot be captured
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    int rc = ensure_queues(ctx, max_descs_per_batch);
+    if (rc != HICR_OK) return rc;
+    HICR_CUDA(ctx, cudaStreamBeginCapture(ctx->stream, cudaStreamCaptureModeRelaxed));
+    ctx->capturing = true;
+    ctx->captured_batches = 0;
+    return HICR_OK;
+}
+
+extern "C" int hicr_graph_end(hicr_ctx_t *ctx, hicr_graph_t **out)
+{
+    if (!ctx || !out) return HICR_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!ctx->capturing) return HICR_ERR_INVALID_ARG;
+    ctx->capturing = false;
+    hicr_graph *g = new hicr_graph();
+    g->ctx = ctx;
+    g->n_batches = ctx->captured_batches;
+    g->n_push = std::min<uint32_t>((uint32_t)ctx->rows.size(), kPushSlots);
+    g->table_version = ctx->table_version;
+    cudaError_t e = cudaStreamEndCapture(ctx->stream, &g->graph);
+    if (e == cudaSuccess && g->graph) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
+    if (e != cudaSuccess || !g->graph) {
+        if (g->graph) cudaGraphDestroy(g->graph);
+        delete g;
+        return cuda_fail(ctx, e == cudaSuccess ? cudaErrorUnknown : e, "hicr_graph_end");
+    }
+    *out = g;
+    return HICR_OK;
+}
+
+extern "C" int hicr_graph_launch(hicr_graph_t *g)
+{
+    if (!g) return HICR_ERR_INVALID_ARG;
+    hicr_ctx *ctx = g->ctx;
+    if (ctx->capturing) return HICR_ERR_BUSY;
+    if (g->table_version != ctx->table_version) return HICR_ERR_INVALID_ARG;   // the recorded launches name another slot table
+    if (g->n_batches == 0) return HICR_OK;
+    HICR_CUDA(ctx, cudaSetDevice(ctx->device));
+    if (ctx->batches_in_epoch + g->n_batches > (uint32_t)kRecRing) {
+        int rc = drain_epoch(ctx, false);
+        if (rc != HICR_OK) return rc;
+    }
+    HICR_CUDA(ctx, cudaGraphLaunch(g->exec, ctx->stream));
+    ctx->launches += g->n_batches;
+    ctx->batch_seq += g->n_batches;
+    ctx->batches_in_epoch += g->n_batches;
+    ctx->epoch_open = true;
+    ctx->last_n_push = g->n_push;
+    ctx->push_stale = false;
+    return HICR_OK;
+}
+
+extern "C" int hicr_graph_destroy(hicr_graph_t *g)
+{
+    if (!g) return HICR_ERR_INVALID_ARG;
+    (void)cudaStreamSynchronize(g->ctx->stream);
+    if (g->exec) cudaGraphExecDestroy(g->exec);
+    if (g->graph) cudaGraphDestroy(g->graph);
+    (void)cudaGetLastError();
+    delete g;
     return HICR_OK;
 }

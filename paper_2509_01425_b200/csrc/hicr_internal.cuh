@@ -113,7 +113,7 @@ struct __align__(16) WorkItem {
     uint64_t pad;
 };
 
-// Device control block of the engine kernel.  All-zero between batches: the last CTA of
+// Device control block of the engine kernel.  All-zero between batches (but for seq): the last CTA of
 // a batch publishes the host record and then clears it, so consecutive batches on the
 // stream reuse it without any memset.  Every word that many CTAs hammer with atomics sits
 // on its own 128-byte line: 2368 warps taking tickets must not delay the grid barrier or
@@ -123,7 +123,8 @@ struct __align__(128) Ctl {
     unsigned long long bad_inv;   // atomicMax of ~((index << 4) | error id); 0 = no error
     unsigned long long t_start;   // %globaltimer at kernel start (CTA 0)
     unsigned long long t_mid;     // %globaltimer after the grid barrier (CTA 0)
-    unsigned int pad0[26];
+    unsigned long long seq;       // batches this context has completed; NOT cleared between batches
+    unsigned int pad0[24];
     // line 1: the grid barrier between validation/binning and the copies, and everything a
     // CTA must know when it leaves it, in ONE word, so that the poll that sees the last
     // arrival also delivers the verdict (no second L2 round trip after the barrier):
@@ -606,6 +607,11 @@ struct hicr_ctx {
     hicr::SlotCnt *d_gdelta = nullptr;       // [HICR_MAX_SLOTS] all-zero between batches
     uint32_t n_global = 0;                   // live rows of kind GLOBAL
     hicr::GlobalTable *globals = nullptr;
+
+    // stream capture of a chain of batches (hicr_graph_*)
+    bool capturing = false;
+    uint32_t captured_batches = 0;
+    uint64_t table_version = 0;              // bumped by every change of the slot table
 
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)

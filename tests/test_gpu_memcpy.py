@@ -9,7 +9,9 @@ import os
 import numpy as np
 import pytest
 
+import oracle
 import workloads as W
+from oracle import Oracle
 from parity import assert_same, run_gpu, run_oracle, to_device_table
 
 pytestmark = pytest.mark.gpu
@@ -599,6 +601,69 @@ def test_fence_async_chain(hicr):
         ctx.fence()
         assert buf.cpu().numpy().tobytes() == ref_imgs[0].tobytes()
         assert ctx.slot_counters(sid) == ref_cnt[-1][0] == (8 * 20000, 8 * 20000)
+
+
+def test_chain_recorded_once_replayed_twice(hicr):
+    """hicr_graph_* (config 4 "as one CUDA graph"): the chain of epochs recorded
+    once and enqueued with one call leaves image and counters as the oracle's epoch-by-epoch run;
+    a second launch replays the same epochs on the image the first one left (the oracle does the
+    same); a replay with a bad descriptor reports it at the fence with its batch index and leaves
+    that batch without effect; recording refuses what it cannot replay."""
+    w = W.chained_epochs(n_epochs=8, n_desc=20000, slot_bytes=32 * W.MiB)
+    imgs = [w.slot_image(0)]
+    o = Oracle()
+    o.slot_register(imgs[0])
+    with _ctx(hicr) as c0:
+        with pytest.raises(hicr.HicrError) as e:
+            c0.graph_begin(16)                                                 # the legacy default stream
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream), hicr.Context(0, stream.cuda_stream) as ctx:
+        buf = torch.from_numpy(w.slot_image(0)).cuda()
+        sid = ctx.slot_register(buf)
+        keep = [to_device_table(e) for e in w.epochs]
+        stream.synchronize()
+        ctx.graph_begin(20000)
+        for t, e in zip(keep, w.epochs):
+            ctx.memcpy_batch(t, n=len(e))
+            ctx.fence_async()
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.memcpy_batch(np.ascontiguousarray(w.epochs[0]))               # a host table cannot be replayed
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence()                                                        # nor can a blocking fence be recorded
+        assert e.value.status == hicr.HICR_ERR_BUSY
+        g = ctx.graph_end()
+        l0 = ctx.launch_count()
+        for rep in (1, 2):
+            for ep in w.epochs:
+                assert o.memcpy_batch(np.ascontiguousarray(ep))[0] == oracle.OK and o.fence() == oracle.OK
+            g.launch()
+            ctx.fence()
+            assert buf.cpu().numpy().tobytes() == imgs[0].tobytes(), "launch %d" % rep
+            assert ctx.slot_counters(sid) == o.slot_counters(0) == (rep * 8 * 20000, rep * 8 * 20000)
+        assert ctx.launch_count() - l0 == 16
+        # a bad descriptor in epoch 5 of the recorded tables: found by the replay, reported at the fence
+        bad = np.ascontiguousarray(w.epochs[5]).copy()
+        bad["size"][777] = 1 << 40
+        keep[5].copy_(to_device_table(bad))
+        for k, ep in enumerate(w.epochs):
+            rc, idx = o.memcpy_batch(bad if k == 5 else np.ascontiguousarray(ep))
+            assert (rc, idx) == ((oracle.ERR_OUT_OF_BOUNDS, 777) if k == 5 else (oracle.OK, None))
+            assert o.fence() == oracle.OK
+        g.launch()
+        with pytest.raises(hicr.HicrError) as e:
+            ctx.fence()
+        assert (e.value.status, e.value.batch_index, e.value.first_bad) == (hicr.HICR_ERR_OUT_OF_BOUNDS, 5, 777)
+        assert buf.cpu().numpy().tobytes() == imgs[0].tobytes()
+        assert ctx.slot_counters(sid) == o.slot_counters(0)
+        # a changed slot table makes the recording stale
+        extra = torch.zeros(16, dtype=torch.uint8, device="cuda")
+        ctx.slot_register(extra)
+        with pytest.raises(hicr.HicrError) as e:
+            g.launch()
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        g.close()
 
 
 def test_fence_expected(hicr):
