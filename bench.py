@@ -54,7 +54,7 @@ def make_workload(name: str, rank: int = 0):
         return W.heavy_tailed("a", seed=seed)
     if name == "heavy_b":
         return W.heavy_tailed("b", seed=seed)
-    if name in ("chain", "chain_async"):
+    if name in ("chain", "chain_async", "chain_graph"):
         return W.chained_epochs(seed=seed)
     raise SystemExit("unknown --config %s" % name)
 
@@ -69,6 +69,9 @@ WORKLOAD_TEXT = {
     "chain": "config 4 chained epochs: 1 slot x 256 MiB, 64 epochs x 65536 descriptors of 8..256 B",
     "chain_async": "config 4 chained epochs with stream-ordered fences (hicr_fence_async) between epochs and ONE blocking "
                    "fence at the end of the timed region (SURVEY.md S8(f) 3)",
+    "chain_graph": "config 4 chained epochs recorded once as ONE CUDA graph of 64 batches (hicr_graph_*) and replayed: one "
+                   "call enqueues 64 epochs, one blocking fence per replay; every replay validates, bins, copies and counts "
+                   "on the device (SURVEY.md S8(f) 3)",
 }
 
 
@@ -102,7 +105,7 @@ class ClockSampler:
         0x80: "hw_power_brake", 0x2: "applications_clocks", 0x100: "display_clock", 0x10: "sync_boost",
     }
 
-    def __init__(self, index: int, period_s: float = 0.005):
+    def __init__(self, index: int, period_s: float = 0.001):
         self.samples, self.reasons, self.period = [], 0, period_s
         self._stop = threading.Event()
         self._thr = None
@@ -191,6 +194,40 @@ def oracle_steps(w, n_steps: int, warmup: int = 0, budget_s: float = None, total
     return times, moved, units
 
 
+def parallel_memcpy_baseline(w, budget_s: float):
+    """The stronger CPU baseline of SURVEY.md S8(d): the same descriptor sets through libc memcpy,
+    descriptors dealt to all host cores this process may use (oracle/parallel_memcpy.c; no
+    validation, no counters -- a timing baseline, not the oracle)."""
+    import oracle
+    cores = host_cores()
+    imgs = [w.slot_image(s) for s in range(len(w.slot_sizes))]
+    sets = [np.ascontiguousarray(e) for e in w.epochs]
+    oracle.parallel_memcpy_batch(imgs, sets[0], cores)            # warm-up (page faults, thread start)
+    t_begin, times, moved = time.perf_counter(), [], []
+    k = 0
+    while time.perf_counter() - t_begin < budget_s:
+        e = sets[k % len(sets)]
+        t0 = time.perf_counter()
+        oracle.parallel_memcpy_batch(imgs, e, cores)
+        times.append(time.perf_counter() - t0)
+        moved.append(2.0 * float(e["size"].sum()))
+        k += 1
+    return {"value": sum(moved) / sum(times) / 1e9, "unit": UNIT, "cores": cores, "kind": "libc memcpy per descriptor, all cores",
+            "sample": "%d full steps of the same workload in %.1f s" % (len(times), sum(times))}
+
+
+def size_decades(sizes):
+    """Index arrays of the descriptors per size decade: [16, 160), [160, 1600), ...."""
+    out, lo = [], 16
+    sizes = np.asarray(sizes)
+    while lo <= int(sizes.max()):
+        idx = np.nonzero((sizes >= lo) & (sizes < 10 * lo))[0]
+        if idx.size:
+            out.append((lo, 10 * lo, idx))
+        lo *= 10
+    return out
+
+
 def bytes_per_step(w) -> float:
     return 2.0 * w.bytes_copied / len(w.epochs)
 
@@ -247,6 +284,50 @@ def pin_rate_gbs(device: int = 0):
         return None
 
 
+def cross_gpu_leg(hicr, ctx, rank, world, group, stream, steps=20, pages=16384, page=4096, timeout_ms=30000):
+    """N > 1 only: every rank volunteers a window as a Global Memory Slot
+     and PUTS `pages` pages of `page` bytes per step into the window of rank + 1
+    (Local-to-Global) with its own copy kernels over the peer mapping; a step ends in
+    the initiator's blocking fence, the leg in one global fence whose count exchange must find
+    every owner's totals.  Returns this rank's numbers; the control plane is `group` (gloo)."""
+    import torch
+    rng = np.random.default_rng(W.BASE_SEED + 7000 + rank)
+    nbytes = pages * page
+    src = torch.from_numpy(rng.integers(0, 256, nbytes, dtype=np.uint8)).cuda()
+    win = torch.zeros(nbytes, dtype=torch.uint8, device="cuda")
+    s_src, s_win = ctx.slot_register(src), ctx.slot_register(win)
+    g = hicr.collective.exchange_global_slots(ctx, 77, [(rank, s_win)], group=group)
+    peer = (rank + 1) % world
+    d = W.make_descs([g[peer]] * pages, [s_src] * pages, rng.permutation(pages).astype(np.uint64) * page,
+                     rng.permutation(pages).astype(np.uint64) * page, [page] * pages)
+    t = torch.from_numpy(d.view(np.uint8).copy()).cuda()
+    for _ in range(3):
+        ctx.memcpy_batch(t, n=pages)
+        ctx.fence()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for _ in range(steps):
+        ctx.memcpy_batch(t, n=pages)
+        ctx.fence()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    t0 = time.perf_counter()
+    hicr.collective.fence_global(ctx, group=group, timeout_ms=timeout_ms)
+    gf_ms = 1e3 * (time.perf_counter() - t0)
+    sent, recv = ctx.global_counters(s_win)
+    # what landed in this rank's window is what rank - 1 put: same seeded source and page permutations
+    prng = np.random.default_rng(W.BASE_SEED + 7000 + (rank - 1) % world)
+    psrc = prng.integers(0, 256, nbytes, dtype=np.uint8).reshape(pages, page)
+    dperm, sperm = prng.permutation(pages), prng.permutation(pages)
+    expect = np.empty_like(psrc)
+    expect[dperm] = psrc[sperm]
+    ok = bool(torch.equal(win.cpu(), torch.from_numpy(expect.reshape(-1))))
+    return {"put_ms_per_step": ms, "put_GBs": 2.0 * nbytes / (ms * 1e-3) / 1e9, "pages": pages, "page_bytes": page,
+            "global_fence_ms": gf_ms, "owner_recv_total": int(recv), "owner_recv_expected": int((steps + 3) * pages),
+            "window_equals_peer_source": ok, "peer": peer}
+
+
 def run_cuda(args):
     import torch
     import paper_2509_01425_b200 as hicr
@@ -293,9 +374,27 @@ def run_cuda(args):
             ctx.memcpy_batch(host_tables[i % n_sets])
             ctx.fence()
 
+        graph = None
+        if args.config == "chain_graph":
+            # the 64 epochs recorded once; a replay = one hicr_graph_launch + one blocking fence
+            ctx.graph_begin(max(n_per))
+            for i in range(n_sets):
+                ctx.memcpy_batch(dev_ptrs[i], n_per[i])
+                ctx.fence_async()
+            graph = ctx.graph_end()
+            K = n_sets * max(1, -(-K // n_sets))      # whole replays only
+
+        def run_steps(k):
+            if graph is None:
+                for i in range(k):
+                    step_device(i)
+            else:
+                for _ in range(max(1, -(-k // n_sets))):
+                    graph.launch()
+                    ctx.fence()
+
         # ---- device-resident arm (value): K steps, nothing else on the stream
-        for i in range(Wm):
-            step_device(i)
+        run_steps(Wm)
         ctx.fence()
         clocks = ClockSampler(local)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -304,15 +403,40 @@ def run_cuda(args):
         clocks.start()
         t_host0 = time.perf_counter()
         e0.record(stream)
-        for i in range(K):
-            step_device(i)
+        run_steps(K)
         ctx.fence()                      # a no-op unless the epochs were closed by stream-ordered fences
         e1.record(stream)
         barrier()
         t_host = time.perf_counter() - t_host0
-        clk = clocks.stop()
+        clk_value_samples = len(clocks.samples)     # the sampler keeps running over the other timed legs below
         launches = ctx.launch_count() - l0
         ms = e0.elapsed_time(e1)
+
+        # ---- spread: every step of a second pass timed on its own with the host clock (a step ends in a
+        # blocking fence, so the host sees its whole duration; CUDA events per step would add ~2 us each)
+        # -- best, median and mean over R >= 20 repetitions -- and the same K steps on ONE
+        # descriptor set (warm: part of the set stays in the 126 MB L2) beside the rotating (cold) ones
+        per_step, warm = None, None
+        if graph is None and args.config != "chain_async":
+            R = max(20, min(K, 400))
+            ts = np.empty(R)
+            for i in range(R):
+                t0 = time.perf_counter()
+                step_device(i)
+                ts[i] = time.perf_counter() - t0
+            per_step = {"repetitions": R, "best_us": 1e6 * float(ts.min()), "median_us": 1e6 * float(np.median(ts)),
+                        "mean_us": 1e6 * float(ts.mean()), "clock": "host, around memcpy_batch + blocking fence"}
+            w0, w1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            for _ in range(3):
+                step_device(0)
+            w0.record(stream)
+            for _ in range(K):
+                step_device(0)
+            w1.record(stream)
+            torch.cuda.synchronize()
+            warm_ms = w0.elapsed_time(w1) / K
+            warm = {"ms_per_step": warm_ms, "value": bytes_per_step(w) / (warm_ms * 1e-3) / 1e9, "unit": UNIT,
+                    "what": "the same descriptor set every step"}
 
         # ---- roofline leg: the same K steps again with the library's CUDA events recorded
         # around every engine-kernel launch on the context's stream (they cost about 2 us per
@@ -325,6 +449,29 @@ def run_cuda(args):
             prof += np.asarray(ctx.profile_read())
         n_prof = K
         ctx.profile_enable(False)
+
+        # ---- config 3: GB/s per size decade -- the descriptors of each decade as a batch of their own
+        per_decade = None
+        if args.config in ("heavy_a", "heavy_b"):
+            per_decade = []
+            for lo, hi, idx in size_decades(host_tables[0]["size"]):
+                sub = np.ascontiguousarray(host_tables[0][idx])
+                t = torch.from_numpy(sub.view(np.uint8).copy()).cuda()
+                reps = 5
+                for _ in range(2):
+                    ctx.memcpy_batch(t, n=len(sub))
+                    ctx.fence()
+                d0, d1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                d0.record(stream)
+                for _ in range(reps):
+                    ctx.memcpy_batch(t, n=len(sub))
+                    ctx.fence()
+                d1.record(stream)
+                torch.cuda.synchronize()
+                dms = d0.elapsed_time(d1) / reps
+                nb = 2.0 * float(sub["size"].sum())
+                per_decade.append({"bytes_from": lo, "bytes_below": hi, "descs": int(len(sub)), "us": 1e3 * dms,
+                                   "GBs": nb / (dms * 1e-3) / 1e9, "descs_per_s": len(sub) / (dms * 1e-3)})
 
         # ---- fence cost alone: an epoch with one 1-descriptor batch
         one = dev_tables[0]
@@ -350,7 +497,30 @@ def run_cuda(args):
         g1.record(stream)
         barrier()
         ms_e2e = g0.elapsed_time(g1)
+        clk = clocks.stop()
+        clk["samples_in_value_leg"] = clk_value_samples
+        clk["covers"] = "value, spread, warm, roofline and end-to-end legs (1 ms period)"
         counters = [ctx.slot_counters(s) for s in ids]
+
+        # ---- N > 1: the cross-GPU put of SURVEY.md S8(e) beside the per-rank number (never inside it)
+        cross = None
+        if world > 1:
+            try:
+                import datetime
+                gloo = dist.new_group(backend="gloo", timeout=datetime.timedelta(seconds=120))
+                ctx.instance_set(rank, world)
+                mine = cross_gpu_leg(hicr, ctx, rank, world, gloo, stream)
+                allr = [None] * world
+                dist.all_gather_object(allr, mine, group=gloo)
+                cross = {"what": "every rank puts 64 MiB per step into the Global Memory Slot of rank + 1 (4 KiB pages, "
+                                 "random permutation), initiator's copy kernels over the CUDA-IPC peer mapping; "
+                                 "unmeasured on hardware until a multi-GPU record exists",
+                         "put_GBs_total": sum(r["put_GBs"] for r in allr), "put_ms_per_step_max": max(r["put_ms_per_step"] for r in allr),
+                         "global_fence_ms_max": max(r["global_fence_ms"] for r in allr),
+                         "counts_ok": all(r["owner_recv_total"] == r["owner_recv_expected"] for r in allr),
+                         "data_ok": all(r["window_equals_peer_source"] for r in allr)}
+            except Exception as exc:
+                cross = {"error": repr(exc)[:300]}
 
     ms_max, ms_e2e_max = rank_max(ms, dist, "cuda"), rank_max(ms_e2e, dist, "cuda")
     bps, dps = bytes_per_step(w), descs_per_step(w)
@@ -385,6 +555,12 @@ def run_cuda(args):
             cpu = {"value": cpu_gbs, "unit": UNIT, "cores": 1, "kind": "oracle",
                    "sample": "%d full steps of the same workload in %.1f s (host cores available: %d)"
                              % (len(times), sum(times), host_cores())}
+        cpu_par = None
+        if not args.no_cpu_baseline:
+            try:
+                cpu_par = parallel_memcpy_baseline(make_workload(args.config, 0), args.cpu_seconds / 2)
+            except Exception as exc:   # a baseline must never cost the line
+                cpu_par = {"error": repr(exc)}
         line = {
             "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": K, "warmup": Wm,
             "ms_per_step": agg["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -393,6 +569,7 @@ def run_cuda(args):
                        "descriptor_tables": "device-resident", "l2": "inputs larger than L2: %d MiB touched per step, "
                        "%d rotating disjoint sets" % (bps / 2 ** 20, n_sets), "sharding": "independent slots per rank"},
             "descs_per_s": agg["descs_per_s"], "fence_us": fence_us, "host_ms_per_step": 1e3 * t_host / K,
+            "per_step": per_step, "warm": warm, "per_size_decade": per_decade,
             "frac_of_hbm_peak": agg["value"] / world / peak,
             "e2e": {"value": agg_e2e["value"], "unit": UNIT,
                     "h2d_bytes_per_step": int(32 * dps), "d2h_bytes_per_step": int(64 + 16 * len(ids)),
@@ -401,9 +578,13 @@ def run_cuda(args):
             "kernel_ms": kernel_ms,
             "roofline": {"bound": "hbm", "kernel": dom, "achieved": achieved, "peak": peak, "unit": UNIT,
                          "frac": achieved / peak, "traffic": traffic, "peak_source": peak_src,
+                         # the same kernel time against the DRAM bytes ncu counted (writes still dirty in L2 at
+                         # kernel end are paid for by the next step): the fraction by bytes actually moved
+                         "frac_by_dram_traffic": (traffic / (kernel_ms[dom] * 1e-3) / 1e9 / peak) if traffic and kernel_ms[dom] > 0 else None,
                          "algorithmic_bytes_per_launch": bps, "pin_rate": pin,
                          "frac_of_pin_rate": (achieved / pin) if pin else None},
-            "cpu_baseline": cpu,
+            "cross_gpu": cross,
+            "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
             "clocks": clk,
             "counters_ok": bool(sum(c[0] for c in counters) == sum(c[1] for c in counters)),
         }

@@ -48,6 +48,14 @@ def main():
             except hicr.HicrError as e:
                 assert e.status == hicr.HICR_ERR_ILLEGAL_DIRECTION
             dist.barrier()                                               # nobody unmaps what a peer still reads
+    # the cross-GPU leg of bench.py --gpus N (N > 1), here between two processes on one GPU
+    import bench
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream), hicr.Context(0, stream.cuda_stream) as ctx:
+        ctx.instance_set(rank, world)
+        r = bench.cross_gpu_leg(hicr, ctx, rank, world, None, stream, steps=3, pages=2048)
+        assert r["window_equals_peer_source"] and r["owner_recv_total"] == r["owner_recv_expected"], r
+        dist.barrier()
     dist.destroy_process_group()
     print("global two-process parity ok (rank %d)" % rank)
 
