@@ -6,6 +6,8 @@
 //                          incoming and outgoing data transfers have been completed"
 #include "hicr_internal.cuh"
 
+#include <sched.h>
+
 #include <algorithm>
 #include <cstdio>
 #include <cstdlib>
@@ -255,7 +257,13 @@ int hicr_init(hicr_ctx_t **out, int device, void *cuda_stream)
             return rc;
         }
     }
-    ctx->stage_pool = stage_pool_create(kStageThreads - 1);   // host threads for host-resident tables, beside the caller's
+    {
+        // host threads for host-resident tables, beside the caller's: half the cores this process may run on
+        cpu_set_t set;
+        CPU_ZERO(&set);
+        int cores = sched_getaffinity(0, sizeof(set), &set) == 0 ? CPU_COUNT(&set) : 1;
+        ctx->stage_pool = stage_pool_create(std::max(1, std::min(kStageThreadsMax, cores / 2)) - 1);
+    }
     *out = ctx;
     return HICR_OK;
 }

@@ -41,7 +41,9 @@ constexpr uint64_t kZeroCopyDescs = 1024;   // host tables up to this many descr
 constexpr unsigned kMaxGroup = 32;         // units per warp ticket, at most (one per lane)
 constexpr unsigned kGss = 3;               // guided self-scheduling: a warp ticket is 1 / (kGss x warps) of what is left
 constexpr unsigned kPrefetchDescs = 2;     // descriptors per warp whose source goes to L2 while the grid barrier fills
-constexpr int kStageThreads = 4;           // host threads that check and stage a host-resident table (caller included)
+constexpr int kStageThreadsMax = 8;        // host threads that check and stage a host-resident table (caller included):
+                                           // half the cores the process may use, at most this many (4 threads: 92 us for the
+                                           // 2 MiB table of config 2, bound by host memory bandwidth)
 
 // error ids packed into Ctl::bad (lower id does not mean higher priority; index decides)
 constexpr unsigned kBadInvalidSlot = 1, kBadOutOfBounds = 2, kBadNoCapacity = 3, kBadDirection = 4;
@@ -584,7 +586,7 @@ struct hicr_ctx {
     // staging of host-resident descriptor tables (returned to `free_stage` at the fence)
     std::vector<hicr::StageBlock> free_stage, used_stage;
 
-    // host threads that check and stage host-resident tables (kStageThreads, the caller included)
+    // host threads that check and stage host-resident tables (up to kStageThreadsMax, the caller included)
     hicr::StagePool *stage_pool = nullptr;
     std::atomic<uint64_t> *stage_done = nullptr;
     uint64_t stage_done_cap = 0;

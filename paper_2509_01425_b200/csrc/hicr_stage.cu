@@ -4,7 +4,7 @@
 //
 // One pass over a 2 MiB table is bound by host memory bandwidth (a plain memcpy of it takes
 // as long as check + copy on one core of the GPU box), so the table is cut into pieces that
-// the caller's thread and kStageThreads - 1 helper threads claim from a shared cursor.  CUDA calls
+// the caller's thread and up to kStageThreadsMax - 1 helper threads claim from a shared cursor.  CUDA calls
 // stay on the caller's thread: it sends every finished prefix of pieces to the device while
 // the others are still being checked.  Helpers spin for a short while after a job (a loop of
 // batches finds them awake) and then sleep on a condition variable.
