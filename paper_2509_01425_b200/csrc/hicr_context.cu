@@ -276,6 +276,7 @@ int hicr_finalize(hicr_ctx_t *ctx)
     stage_pool_destroy(ctx->stage_pool);
     stage_done_free(ctx->stage_done);
     global_teardown(ctx);
+    launch_cache_free(ctx);
     cudaFree(ctx->d_slots);
     cudaFree(ctx->d_cnt);
     cudaFree(ctx->d_ctl);

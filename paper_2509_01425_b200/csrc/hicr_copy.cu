@@ -691,6 +691,90 @@ int engine_setup(hicr_ctx *ctx)
     return HICR_OK;
 }
 
+// ---- launching the engine kernel.  A one-node CUDA graph that is already instantiated starts
+// about 3 us sooner than the same cooperative launch through cudaLaunchCooperativeKernel (config 2:
+// 97.7 against 100.4-101.2 us per step; the front end replays a command buffer it has seen), so the
+// context keeps a few instantiated one-kernel graphs, looks the launch up by its arguments, and
+// rewrites the node's parameters of the least recently used one when none matches.  Nothing about
+// the batch is cached: every launch runs validation, binning, copies and counters.
+constexpr int kLaunchSlots = 8;
+struct LaunchSlot {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    cudaGraphNode_t node = nullptr;
+    EngineArgs args;
+    unsigned grid = 0;
+    size_t smem = 0;
+    uint64_t used = 0;
+};
+struct LaunchCache {
+    LaunchSlot slot[kLaunchSlots];
+    uint64_t clock = 0;
+    bool broken = false;   // graph path refused once: plain launches from then on
+};
+
+void launch_cache_free(hicr_ctx *ctx)
+{
+    LaunchCache *c = static_cast<LaunchCache *>(ctx->launch_cache);
+    if (!c) return;
+    for (auto &s : c->slot) {
+        if (s.exec) cudaGraphExecDestroy(s.exec);
+        if (s.graph) cudaGraphDestroy(s.graph);
+    }
+    delete c;
+    ctx->launch_cache = nullptr;
+}
+
+static cudaError_t launch_engine(hicr_ctx *ctx, EngineArgs &a, unsigned grid, size_t smem)
+{
+    void *args[] = {&a};
+    if (!ctx->launch_cache) ctx->launch_cache = new LaunchCache();
+    LaunchCache *c = static_cast<LaunchCache *>(ctx->launch_cache);
+    if (c->broken)
+        return cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args, smem, ctx->stream);
+    LaunchSlot *hit = nullptr, *lru = &c->slot[0];
+    for (auto &s : c->slot) {
+        if (s.exec && s.grid == grid && s.smem == smem && memcmp(&s.args, &a, sizeof(EngineArgs)) == 0) hit = &s;
+        if (s.used < lru->used) lru = &s;
+    }
+    if (!hit) {
+        cudaKernelNodeParams p = {};
+        p.func = (void *)engine_kernel;
+        p.gridDim = dim3(grid);
+        p.blockDim = dim3(kThreads);
+        p.sharedMemBytes = (unsigned)smem;
+        p.kernelParams = args;
+        cudaError_t e = cudaSuccess;
+        if (lru->exec) {
+            e = cudaGraphExecKernelNodeSetParams(lru->exec, lru->node, &p);
+        } else {
+            e = cudaGraphCreate(&lru->graph, 0);
+            if (e == cudaSuccess) e = cudaGraphAddKernelNode(&lru->node, lru->graph, nullptr, 0, &p);
+            if (e == cudaSuccess) {
+                cudaKernelNodeAttrValue v;
+                memset(&v, 0, sizeof(v));
+                v.cooperative = 1;   // the grid barrier needs every CTA resident
+                e = cudaGraphKernelNodeSetAttribute(lru->node, cudaKernelNodeAttributeCooperative, &v);
+            }
+            if (e == cudaSuccess) e = cudaGraphInstantiate(&lru->exec, lru->graph, 0);
+        }
+        if (e != cudaSuccess) {
+            (void)cudaGetLastError();
+            if (lru->exec) cudaGraphExecDestroy(lru->exec);
+            if (lru->graph) cudaGraphDestroy(lru->graph);
+            *lru = LaunchSlot();
+            c->broken = true;
+            return cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args, smem, ctx->stream);
+        }
+        memcpy(&lru->args, &a, sizeof(EngineArgs));
+        lru->grid = grid;
+        lru->smem = smem;
+        hit = lru;
+    }
+    hit->used = ++c->clock;
+    return cudaGraphLaunch(hit->exec, ctx->stream);
+}
+
 }  // namespace hicr
 
 using namespace hicr;
@@ -752,6 +836,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
     }
 
     EngineArgs a;
+    memset(&a, 0, sizeof(a));   // (padding included: launches are looked up by these bytes)
     a.descs = d_descs;
     a.n = n;
     a.slots = ctx->d_slots;
@@ -781,8 +866,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         return HICR_OK;   // the context's books are kept by hicr_graph_launch
     }
     if (ctx->profiling) HICR_CUDA(ctx, cudaEventRecord(ctx->ev[0], ctx->stream));
-    HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args,
-                                               engine_smem_bytes(a.n_slots), ctx->stream));
+    HICR_CUDA(ctx, launch_engine(ctx, a, grid, engine_smem_bytes(a.n_slots)));
     ctx->launches++;
     if (ctx->profiling) {
         HICR_CUDA(ctx, cudaEventRecord(ctx->ev[1], ctx->stream));

@@ -615,6 +615,8 @@ struct hicr_ctx {
     uint32_t captured_batches = 0;
     uint64_t table_version = 0;              // bumped by every change of the slot table
 
+    void *launch_cache = nullptr;            // hicr_copy.cu: instantiated one-kernel graphs of recent engine launches
+
     uint64_t launches = 0;
     int engine_grid = 0;                     // co-resident CTAs of the engine kernel (cooperative launch)
     uint32_t tma_min = hicr::kTmaMinDefault; // HICR_TMA_MIN environment override (0xffffffff = bulk path off)
@@ -632,6 +634,7 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what);
 int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
 int engine_setup(hicr_ctx *ctx);
+void launch_cache_free(hicr_ctx *ctx);
 int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const StageBlock &b, uint64_t *first_bad,
                 int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
 int bad_to_status(unsigned id);
