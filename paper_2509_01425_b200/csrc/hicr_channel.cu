@@ -29,6 +29,8 @@ struct hicr_channel {
     hicr::ChannelState *d_state = nullptr;
     unsigned int *d_ticket = nullptr;
     uint64_t head = 0, tail = 0;   // host mirror as of the last completed call
+    hicr::NodeLauncher call[2];    // one-kernel graphs of the host-call push (0) and pop (1)
+    bool call_plain = false;       // the graph path was refused once
     // device scratch of the device-resident runs, kept between calls (grown on demand)
     unsigned char *d_tab = nullptr;
     size_t tab_bytes = 0;
@@ -437,6 +439,8 @@ int hicr_channel_destroy(hicr_channel_t *ch)
     (void)cudaStreamSynchronize(ch->ctx->stream);
     cudaFree(ch->d_state);
     cudaFree(ch->d_tab);
+    node_free(ch->call[0]);
+    node_free(ch->call[1]);
     ch->ctx->ring_refs[ch->ring]--;
     delete ch;
     return HICR_OK;
@@ -472,12 +476,27 @@ static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uin
     CallResult *res = ctx->d_call;
     const unsigned long long seq = ++ctx->call_seq;
     SlotCnt *cl = ctx->d_cnt + li, *cr = ctx->d_cnt + ch->ring;
-    if (push)
-        channel_call_kernel<true><<<grid, kCallThreads, 0, ctx->stream>>>(
-            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->sent, &cr->recv, res, seq);
-    else
-        channel_call_kernel<false><<<grid, kCallThreads, 0, ctx->stream>>>(
-            ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->recv, &cr->sent, res, seq);
+    // (one-kernel graph with rewritten parameters: starts sooner than a stream launch, see NodeLauncher)
+    bool launched = false;
+    if (!ch->call_plain) {
+        ChannelState *st = ch->d_state;
+        unsigned int *tk = ch->d_ticket;
+        uint64_t T = ch->T, C = ch->C, room = lsize - off, nn = n;
+        unsigned long long *c_lin = push ? &cl->sent : &cl->recv, *c_ring = push ? &cr->recv : &cr->sent, sq = seq;
+        void *args[] = {&st, &tk, &ring, &T, &C, &lin, &room, &nn, &c_lin, &c_ring, &res, &sq};
+        const void *fn = push ? (const void *)channel_call_kernel<true> : (const void *)channel_call_kernel<false>;
+        launched = node_launch(ch->call[push ? 0 : 1], fn, dim3(grid), dim3(kCallThreads), 0, args, false, true, ctx->stream) ==
+                   cudaSuccess;
+        if (!launched) ch->call_plain = true;
+    }
+    if (!launched) {
+        if (push)
+            channel_call_kernel<true><<<grid, kCallThreads, 0, ctx->stream>>>(
+                ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->sent, &cr->recv, res, seq);
+        else
+            channel_call_kernel<false><<<grid, kCallThreads, 0, ctx->stream>>>(
+                ch->d_state, ch->d_ticket, ring, ch->T, ch->C, lin, lsize - off, n, &cl->recv, &cr->sent, res, seq);
+    }
     ctx->launches++;
     ctx->push_stale = true;   // the device counters moved after the last batch's pushed snapshot
     HICR_CUDA(ctx, cudaGetLastError());

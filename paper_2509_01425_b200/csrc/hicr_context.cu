@@ -24,6 +24,44 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what)
     return HICR_ERR_CUDA;
 }
 
+cudaError_t node_launch(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
+                        bool update, cudaStream_t stream)
+{
+    cudaKernelNodeParams p = {};
+    p.func = const_cast<void *>(func);
+    p.gridDim = grid;
+    p.blockDim = block;
+    p.sharedMemBytes = (unsigned)smem;
+    p.kernelParams = args;
+    cudaError_t e = cudaSuccess;
+    if (!l.exec) {
+        e = cudaGraphCreate(&l.graph, 0);
+        if (e == cudaSuccess) e = cudaGraphAddKernelNode(&l.node, l.graph, nullptr, 0, &p);
+        if (e == cudaSuccess && cooperative) {
+            cudaKernelNodeAttrValue v;
+            memset(&v, 0, sizeof(v));
+            v.cooperative = 1;
+            e = cudaGraphKernelNodeSetAttribute(l.node, cudaKernelNodeAttributeCooperative, &v);
+        }
+        if (e == cudaSuccess) e = cudaGraphInstantiate(&l.exec, l.graph, 0);
+    } else if (update) {
+        e = cudaGraphExecKernelNodeSetParams(l.exec, l.node, &p);
+    }
+    if (e != cudaSuccess) {
+        (void)cudaGetLastError();
+        node_free(l);
+        return e;
+    }
+    return cudaGraphLaunch(l.exec, stream);
+}
+
+void node_free(NodeLauncher &l)
+{
+    if (l.exec) cudaGraphExecDestroy(l.exec);
+    if (l.graph) cudaGraphDestroy(l.graph);
+    l = NodeLauncher();
+}
+
 int bad_to_status(unsigned id)
 {
     switch (id) {

@@ -699,9 +699,7 @@ int engine_setup(hicr_ctx *ctx)
 // the batch is cached: every launch runs validation, binning, copies and counters.
 constexpr int kLaunchSlots = 8;
 struct LaunchSlot {
-    cudaGraph_t graph = nullptr;
-    cudaGraphExec_t exec = nullptr;
-    cudaGraphNode_t node = nullptr;
+    NodeLauncher node;
     EngineArgs args;
     unsigned grid = 0;
     size_t smem = 0;
@@ -710,17 +708,14 @@ struct LaunchSlot {
 struct LaunchCache {
     LaunchSlot slot[kLaunchSlots];
     uint64_t clock = 0;
-    bool broken = false;   // graph path refused once: plain launches from then on
+    bool broken = false;   // the graph path was refused once: stream launches from then on
 };
 
 void launch_cache_free(hicr_ctx *ctx)
 {
     LaunchCache *c = static_cast<LaunchCache *>(ctx->launch_cache);
     if (!c) return;
-    for (auto &s : c->slot) {
-        if (s.exec) cudaGraphExecDestroy(s.exec);
-        if (s.graph) cudaGraphDestroy(s.graph);
-    }
+    for (auto &s : c->slot) node_free(s.node);
     delete c;
     ctx->launch_cache = nullptr;
 }
@@ -730,49 +725,25 @@ static cudaError_t launch_engine(hicr_ctx *ctx, EngineArgs &a, unsigned grid, si
     void *args[] = {&a};
     if (!ctx->launch_cache) ctx->launch_cache = new LaunchCache();
     LaunchCache *c = static_cast<LaunchCache *>(ctx->launch_cache);
-    if (c->broken)
-        return cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args, smem, ctx->stream);
-    LaunchSlot *hit = nullptr, *lru = &c->slot[0];
-    for (auto &s : c->slot) {
-        if (s.exec && s.grid == grid && s.smem == smem && memcmp(&s.args, &a, sizeof(EngineArgs)) == 0) hit = &s;
-        if (s.used < lru->used) lru = &s;
-    }
-    if (!hit) {
-        cudaKernelNodeParams p = {};
-        p.func = (void *)engine_kernel;
-        p.gridDim = dim3(grid);
-        p.blockDim = dim3(kThreads);
-        p.sharedMemBytes = (unsigned)smem;
-        p.kernelParams = args;
-        cudaError_t e = cudaSuccess;
-        if (lru->exec) {
-            e = cudaGraphExecKernelNodeSetParams(lru->exec, lru->node, &p);
-        } else {
-            e = cudaGraphCreate(&lru->graph, 0);
-            if (e == cudaSuccess) e = cudaGraphAddKernelNode(&lru->node, lru->graph, nullptr, 0, &p);
-            if (e == cudaSuccess) {
-                cudaKernelNodeAttrValue v;
-                memset(&v, 0, sizeof(v));
-                v.cooperative = 1;   // the grid barrier needs every CTA resident
-                e = cudaGraphKernelNodeSetAttribute(lru->node, cudaKernelNodeAttributeCooperative, &v);
-            }
-            if (e == cudaSuccess) e = cudaGraphInstantiate(&lru->exec, lru->graph, 0);
+    if (!c->broken) {
+        LaunchSlot *hit = nullptr, *lru = &c->slot[0];
+        for (auto &s : c->slot) {
+            if (s.node.exec && s.grid == grid && s.smem == smem && memcmp(&s.args, &a, sizeof(EngineArgs)) == 0) hit = &s;
+            if (s.used < lru->used) lru = &s;
         }
-        if (e != cudaSuccess) {
-            (void)cudaGetLastError();
-            if (lru->exec) cudaGraphExecDestroy(lru->exec);
-            if (lru->graph) cudaGraphDestroy(lru->graph);
-            *lru = LaunchSlot();
-            c->broken = true;
-            return cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args, smem, ctx->stream);
+        LaunchSlot *use = hit ? hit : lru;
+        cudaError_t e = node_launch(use->node, (const void *)engine_kernel, dim3(grid), dim3(kThreads), smem, args, true, !hit,
+                                    ctx->stream);
+        if (e == cudaSuccess) {
+            memcpy(&use->args, &a, sizeof(EngineArgs));
+            use->grid = grid;
+            use->smem = smem;
+            use->used = ++c->clock;
+            return e;
         }
-        memcpy(&lru->args, &a, sizeof(EngineArgs));
-        lru->grid = grid;
-        lru->smem = smem;
-        hit = lru;
+        c->broken = true;
     }
-    hit->used = ++c->clock;
-    return cudaGraphLaunch(hit->exec, ctx->stream);
+    return cudaLaunchCooperativeKernel((const void *)engine_kernel, dim3(grid), dim3(kThreads), args, smem, ctx->stream);
 }
 
 }  // namespace hicr
