@@ -54,6 +54,8 @@ def make_workload(name: str, rank: int = 0):
         return W.heavy_tailed("a", seed=seed)
     if name == "heavy_b":
         return W.heavy_tailed("b", seed=seed)
+    if name == "heavy_b_aligned":
+        return W.heavy_tailed("b", seed=seed, align=16)
     if name in ("chain", "chain_async", "chain_graph"):
         return W.chained_epochs(seed=seed)
     raise SystemExit("unknown --config %s" % name)
@@ -66,6 +68,8 @@ WORKLOAD_TEXT = {
     "tiny": "config 1 tiny: 2 slots x 1 MiB, 256 descriptors of 1..4096 B, 1 fence per step",
     "heavy_a": "config 3a heavy-tailed: 64 slots x 256 MiB, 100000 descriptors, power law 1.3 on 16 B..16 MiB",
     "heavy_b": "config 3b heavy-tailed: 64 slots x 256 MiB, log-uniform 16 B..16 MiB until full",
+    "heavy_b_aligned": "config 3b with offsets and sizes rounded down to multiples of 16 B (NOT a BASELINE config: every "
+                       "chunk is eligible for the bulk-copy path; run with HICR_TMA_MIN=0xffffffff for the vector path)",
     "chain": "config 4 chained epochs: 1 slot x 256 MiB, 64 epochs x 65536 descriptors of 8..256 B",
     "chain_async": "config 4 chained epochs with stream-ordered fences (hicr_fence_async) between epochs and ONE blocking "
                    "fence at the end of the timed region (SURVEY.md S8(f) 3)",
@@ -98,56 +102,82 @@ def rank_max(x: float, dist=None, device="cpu") -> float:
 
 # --------------------------------------------------------------------------- clocks
 class ClockSampler:
-    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+    """Samples SM clock and throttle reasons through NVML while the timed legs run -- in a process
+    of its own: a sampling THREAD takes the interpreter lock for tens of microseconds per sample,
+    which a 2 ms timed region of 100 us steps pays for (5 us per step at 20 steps).  The child
+    stamps every sample with the wall clock; the parent keeps those that fall into its windows."""
 
     REASONS = {
         0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
         0x80: "hw_power_brake", 0x2: "applications_clocks", 0x100: "display_clock", 0x10: "sync_boost",
     }
-
-    def __init__(self, index: int, period_s: float = 0.001):
-        self.samples, self.reasons, self.period = [], 0, period_s
-        self._stop = threading.Event()
-        self._thr = None
-        self.max_mhz = None
+    CHILD = r"""
+import sys, time
+import pynvml as nv
+nv.nvmlInit()
+h = nv.nvmlDeviceGetHandleByIndex(int(sys.argv[1]))
+period = float(sys.argv[2])
+print("max %d" % nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM), flush=True)
+while True:
+    try:
+        r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+    except Exception:
         try:
-            import pynvml
-            pynvml.nvmlInit()
-            self._nv = pynvml
-            self._h = pynvml.nvmlDeviceGetHandleByIndex(index)
-            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self._h, pynvml.NVML_CLOCK_SM)
+            r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
         except Exception:
-            self._nv = None
+            r = 0
+    print("%.6f %d %d" % (time.time(), nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM), r), flush=True)
+    time.sleep(period)
+"""
 
-    def _run(self):
-        nv = self._nv
-        while not self._stop.is_set():
-            try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self._h, nv.NVML_CLOCK_SM))
-                self.reasons |= int(nv.nvmlDeviceGetCurrentClocksEventReasons(self._h))
-            except Exception:
-                try:
-                    self.reasons |= int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(self._h))
-                except Exception:
-                    pass
-            self._stop.wait(self.period)
+    def __init__(self, index: int, period_s: float = 0.0002):
+        import subprocess
+        self.max_mhz, self._proc, self._t0 = None, None, None
+        try:
+            self._proc = subprocess.Popen([sys.executable, "-c", self.CHILD, str(index), str(period_s)],
+                                          stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            first = self._proc.stdout.readline().split()          # the child is up and sampling from here on
+            self.max_mhz = int(first[1]) if len(first) == 2 and first[0] == "max" else None
+        except Exception:
+            self._proc = None
 
     def start(self):
-        if self._nv:
-            self._thr = threading.Thread(target=self._run, daemon=True)
-            self._thr.start()
+        self._t0 = time.time()
 
-    def stop(self):
-        if self._thr:
-            self._stop.set()
-            self._thr.join()
-        names = sorted(n for bit, n in self.REASONS.items() if self.reasons & bit)
-        return {
-            "sm_mhz": float(np.median(self.samples)) if self.samples else None,
+    def mark(self):
+        """End of a window that began at start(); returns its (t0, t1)."""
+        return (self._t0, time.time())
+
+    def stop(self, windows=None):
+        """Ends the child; the summary covers start() .. now, plus a sample count per named window."""
+        t1 = time.time()
+        rows = []
+        if self._proc:
+            time.sleep(0.003)                                       # let the last samples through the pipe
+            self._proc.terminate()
+            try:
+                out, _ = self._proc.communicate(timeout=5)
+            except Exception:
+                self._proc.kill()
+                out = ""
+            for line in out.splitlines():
+                f = line.split()
+                if len(f) == 3:
+                    rows.append((float(f[0]), int(f[1]), int(f[2])))
+        t0 = self._t0 if self._t0 is not None else 0.0
+        inside = [r for r in rows if t0 <= r[0] <= t1]
+        reasons = 0
+        for r in inside:
+            reasons |= r[2]
+        res = {
+            "sm_mhz": float(np.median([r[1] for r in inside])) if inside else None,
             "sm_max_mhz": self.max_mhz,
-            "reasons": names,
-            "samples": len(self.samples),
+            "reasons": sorted(n for bit, n in self.REASONS.items() if reasons & bit),
+            "samples": len(inside),
         }
+        for name, (a, b) in (windows or {}).items():
+            res["samples_in_" + name] = sum(1 for r in rows if a <= r[0] <= b)
+        return res
 
 
 # --------------------------------------------------------------------------- CPU oracle arm
@@ -351,8 +381,10 @@ def run_cuda(args):
 
     w = make_workload(args.config, rank)
     stream = torch.cuda.Stream()
-    K, Wm = args.steps, max(3, args.warmup)
     n_sets = len(w.epochs)
+    # at least 3 warm-up steps, and every rotating descriptor set once (the first use of a set is not a
+    # steady-state step: cold TLB entries for its pages, the launch of a table not seen before)
+    K, Wm = args.steps, max(3, args.warmup, n_sets if n_sets <= 8 else 3)
     with torch.cuda.stream(stream):
         ctx = hicr.Context(local, stream.cuda_stream)
         bufs = [torch.from_numpy(w.slot_image(s)).to("cuda", non_blocking=False) for s in range(len(w.slot_sizes))]
@@ -408,7 +440,7 @@ def run_cuda(args):
         e1.record(stream)
         barrier()
         t_host = time.perf_counter() - t_host0
-        clk_value_samples = len(clocks.samples)     # the sampler keeps running over the other timed legs below
+        clk_value_window = clocks.mark()            # the sampler keeps running over the other timed legs below
         launches = ctx.launch_count() - l0
         ms = e0.elapsed_time(e1)
 
@@ -452,7 +484,7 @@ def run_cuda(args):
 
         # ---- config 3: GB/s per size decade -- the descriptors of each decade as a batch of their own
         per_decade = None
-        if args.config in ("heavy_a", "heavy_b"):
+        if args.config in ("heavy_a", "heavy_b", "heavy_b_aligned"):
             per_decade = []
             for lo, hi, idx in size_decades(host_tables[0]["size"]):
                 sub = np.ascontiguousarray(host_tables[0][idx])
@@ -497,9 +529,8 @@ def run_cuda(args):
         g1.record(stream)
         barrier()
         ms_e2e = g0.elapsed_time(g1)
-        clk = clocks.stop()
-        clk["samples_in_value_leg"] = clk_value_samples
-        clk["covers"] = "value, spread, warm, roofline and end-to-end legs (1 ms period)"
+        clk = clocks.stop({"value_leg": clk_value_window})
+        clk["covers"] = "value, spread, warm, roofline and end-to-end legs (0.2 ms period, sampled by a separate process)"
         counters = [ctx.slot_counters(s) for s in ids]
 
         # ---- N > 1: the cross-GPU put of SURVEY.md S8(e) beside the per-rank number (never inside it)

@@ -24,8 +24,8 @@ int cuda_fail(hicr_ctx *ctx, cudaError_t e, const char *what)
     return HICR_ERR_CUDA;
 }
 
-cudaError_t node_launch(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
-                        bool update, cudaStream_t stream)
+cudaError_t node_prepare(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
+                         bool update)
 {
     cudaKernelNodeParams p = {};
     p.func = const_cast<void *>(func);
@@ -50,9 +50,15 @@ cudaError_t node_launch(NodeLauncher &l, const void *func, dim3 grid, dim3 block
     if (e != cudaSuccess) {
         (void)cudaGetLastError();
         node_free(l);
-        return e;
     }
-    return cudaGraphLaunch(l.exec, stream);
+    return e;
+}
+
+cudaError_t node_launch(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
+                        bool update, cudaStream_t stream)
+{
+    cudaError_t e = node_prepare(l, func, grid, block, smem, args, cooperative, update);
+    return e == cudaSuccess ? cudaGraphLaunch(l.exec, stream) : e;
 }
 
 void node_free(NodeLauncher &l)

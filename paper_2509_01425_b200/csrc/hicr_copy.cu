@@ -723,7 +723,16 @@ void launch_cache_free(hicr_ctx *ctx)
 static cudaError_t launch_engine(hicr_ctx *ctx, EngineArgs &a, unsigned grid, size_t smem)
 {
     void *args[] = {&a};
-    if (!ctx->launch_cache) ctx->launch_cache = new LaunchCache();
+    if (!ctx->launch_cache) {
+        // all slots are instantiated now (about 50 us each, once per context), so that a launch that
+        // matches none of them later costs a parameter rewrite, not an instantiation
+        LaunchCache *fresh = new LaunchCache();
+        for (auto &s : fresh->slot)
+            if (!fresh->broken && node_prepare(s.node, (const void *)engine_kernel, dim3(grid), dim3(kThreads), smem, args, true, false) !=
+                                      cudaSuccess)
+                fresh->broken = true;
+        ctx->launch_cache = fresh;
+    }
     LaunchCache *c = static_cast<LaunchCache *>(ctx->launch_cache);
     if (!c->broken) {
         LaunchSlot *hit = nullptr, *lru = &c->slot[0];

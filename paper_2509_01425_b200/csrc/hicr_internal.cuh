@@ -549,6 +549,8 @@ struct NodeLauncher {
 };
 // Launch `func` through the launcher: builds it on first use, rewrites the node's parameters when
 // `update`, then cudaGraphLaunch.  A failure to build or update is returned (the caller falls back).
+cudaError_t node_prepare(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
+                         bool update);
 cudaError_t node_launch(NodeLauncher &l, const void *func, dim3 grid, dim3 block, size_t smem, void **args, bool cooperative,
                         bool update, cudaStream_t stream);
 void node_free(NodeLauncher &l);

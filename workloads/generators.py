@@ -147,7 +147,7 @@ def _power_law_sizes(rng, n, a, b, alpha):
 
 def heavy_tailed(variant: str = "a", n_slots: int = 64, slot_bytes: int = 256 * MiB,
                  src_zone: int = 32 * MiB, n_desc: int = 100000, smin: int = 16, smax: int = 16 * MiB,
-                 alpha: float = 1.3, seed: int = BASE_SEED) -> CopyWorkload:
+                 alpha: float = 1.3, seed: int = BASE_SEED, align: int = 1) -> CopyWorkload:
     """Config 3 (reading 19: BASELINE.json's literal text needs 112.7 GiB of disjoint
     destinations inside 16 GiB, so two variants are run).
 
@@ -158,7 +158,10 @@ def heavy_tailed(variant: str = "a", n_slots: int = 64, slot_bytes: int = 256 * 
 
       'a': n_desc sizes from the truncated power law p(s) ~ s^-alpha on [smin, smax].
       'b': literal log-uniform sizes floor(smin * 2^(log2(smax/smin) u)), taken in draw
-           order until no slot has room for the next one (at most n_desc)."""
+           order until no slot has room for the next one (at most n_desc).
+
+    ``align`` > 1 (not a BASELINE config; used to measure the bulk-copy path): offsets and sizes
+    rounded DOWN to multiples of ``align`` afterwards, which keeps the ranges disjoint."""
     rng = rng_for(3, 0 if variant == "a" else 1, seed)
     room = np.full(n_slots, slot_bytes - src_zone, dtype=np.int64)
     if variant == "a":
@@ -187,8 +190,12 @@ def heavy_tailed(variant: str = "a", n_slots: int = 64, slot_bytes: int = 256 * 
     for s in range(n_slots):
         idx = np.nonzero(dst_slot == s)[0]
         dst_off[idx] = gaps_composition(rng, size[idx], src_zone, slot_bytes)
+    if align > 1:
+        size = np.maximum(size // align * align, align)
+        src_off = src_off // align * align
+        dst_off = dst_off // np.uint64(align) * np.uint64(align)
     d = make_descs(dst_slot, src_slot, dst_off, src_off, size)
-    return CopyWorkload("heavy_tailed_3" + variant, 3, [slot_bytes] * n_slots, [d], seed,
+    return CopyWorkload("heavy_tailed_3" + variant + ("_aligned%d" % align if align > 1 else ""), 3, [slot_bytes] * n_slots, [d], seed,
                         {"variant": variant, "alpha": alpha if variant == "a" else 1.0, "src_zone": src_zone})
 
 
