@@ -220,6 +220,44 @@ def test_spsc_stream_equals_call_sequence(hicr, T, C, N, maxb):
         p.close()
 
 
+@pytest.mark.parametrize("T,C,pre,batches", [
+    (256, 1024, 37, [0, 5, 0, 3000, 1, 0, 1024, 2047, 0]),      # pushes of zero tokens, pushes larger than the ring
+    (64, 48, 5, [100, 1, 1, 48, 49, 7]),                        # capacity not a power of two: pieces of 16 tokens
+    (4096, 8, 3, [1, 30, 2, 9]),                                # two tokens per piece
+    (16384, 4, 1, [5, 11]),                                     # a token larger than the default stage
+    (32, 1024, 9, [4000, 96]),                                  # 1 KiB pieces: the smallest the pipeline takes
+    (16, 64, 2, [500]),                                         # pieces below 1 KiB: the vector kernels
+])
+def test_stream_from_a_ring_in_use(hicr, T, C, pre, batches):
+    """hicr_channel_stream on a channel whose counters are not at zero (host pushes / pops first, so
+    the first piece starts inside a piece boundary), with the batch shapes above: sink, ring,
+    head / tail and counters as the oracle's call sequence; then host calls again."""
+    N = sum(batches)
+    rng = np.random.default_rng(T + C)
+    p = Pair(hicr, T, C, rng.integers(0, 256, (pre + N + 2) * T, dtype=np.uint8), (pre + N + 2) * T)
+    try:
+        for i in range(pre):                                     # one token in, one out: head = tail = pre
+            assert p.ch.push(p.ids[1], i * T, 1) == 1 == p.o.channel_push(p.och, p.ids[1], i * T, 1)[1]
+            assert p.ch.pop(p.ids[2], i * T, 1) == 1 == p.o.channel_pop(p.och, p.ids[2], i * T, 1)[1]
+        pos = pre
+        for b in batches:
+            left = b
+            while left:
+                rc, k = p.o.channel_push(p.och, p.ids[1], pos * T, left)
+                assert rc == oracle.OK and k > 0
+                assert p.o.channel_pop(p.och, p.ids[2], pos * T, C) == (oracle.OK, k)
+                pos += k
+                left -= k
+        p.ch.stream(p.ids[1], pre * T, p.ids[2], pre * T, batches)
+        p.check("stream from head = tail = %d" % pre)
+        assert p.ch.counters() == (pre + N, pre + N)
+        assert p.ch.push(p.ids[1], pos * T, 2) == min(2, C) == p.o.channel_push(p.och, p.ids[1], pos * T, 2)[1]
+        assert p.ch.pop(p.ids[2], pos * T, 2) == min(2, C) == p.o.channel_pop(p.och, p.ids[2], pos * T, 2)[1]
+        p.check("after the run")
+    finally:
+        p.close()
+
+
 def _mpsc_both(hicr, w, max_batch):
     T, C, P, N = w.token_bytes, w.capacity, w.producers, w.n_tokens
     # oracle: P independent SPSC channels driven in the seeded interleaving
