@@ -238,7 +238,8 @@ int hicr_global_volunteer(hicr_ctx_t *ctx, uint64_t tag, uint64_t key, hicr_slot
  * (tag, key) exists already in this context, HICR_ERR_INVALID_ARG on a handle that is not one
  * (or of another tag), HICR_ERR_UNSUPPORTED_SPACE if an owner's memory cannot be mapped from this
  * device ("Otherwise, it will be rejected"), HICR_ERR_NO_CAPACITY; then no slot is
- * created.  n == 0 is a valid (empty) exchange.  hicr_slot_unregister drops a global slot again. */
+ * created.  n == 0 is a valid (empty) exchange.  hicr_slot_unregister drops a global slot again;
+ * an owner keeps its storage and its context alive until every instance has dropped the slot. */
 int hicr_global_exchange(hicr_ctx_t *ctx, uint64_t tag, const hicr_global_handle_t *handles, uint64_t n,
                          hicr_slot_t *out_slots);
 

@@ -297,9 +297,11 @@ class Context:
             self._fail(rc, "hicr_global_lookup")
         return out.value
 
-    def global_fence_begin(self) -> np.ndarray:
+    def global_fence_begin(self, defer_error: bool = False):
         """hicr_global_fence_begin: the blocking local fence, then this context's lines of the
-        count exchange (GLOBAL_COUNT_DTYPE)."""
+        count exchange (GLOBAL_COUNT_DTYPE).  A deferred error of the epoch is raised here, or --
+        ``defer_error`` -- returned as the second element of (lines, HicrError or None), so that a
+        collective caller can finish the exchange with its peers before raising it."""
         cap = 64
         while True:
             out = np.zeros(cap, dtype=GLOBAL_COUNT_DTYPE)
@@ -308,11 +310,16 @@ class Context:
             if rc == HICR_ERR_NO_CAPACITY and n.value > cap:
                 cap = int(n.value)
                 continue
+            err = None
             if rc != HICR_OK:
                 b, i = ctypes.c_uint64(), ctypes.c_uint64()
                 lib.hicr_fence_error(self._h, ctypes.byref(b), ctypes.byref(i))
-                self._fail(rc, "hicr_global_fence_begin", first_bad=i.value, batch_index=b.value)
-            return out[: n.value].copy()
+                detail = lib.hicr_last_cuda_error(self._h).decode() if rc == HICR_ERR_CUDA else ""
+                err = HicrError(rc, "hicr_global_fence_begin", first_bad=i.value, batch_index=b.value, detail=detail)
+                if not defer_error or rc == HICR_ERR_CUDA:
+                    raise err
+            lines = out[: n.value].copy()
+            return (lines, err) if defer_error else lines
 
     def global_fence_end(self, all_counts: np.ndarray, timeout_ms: int = 0):
         a = np.ascontiguousarray(all_counts, dtype=GLOBAL_COUNT_DTYPE)

@@ -45,9 +45,11 @@ def fence_global(ctx: Context, group=None, timeout_ms: int = 0) -> None:
     every instance tells every other what it initiated on each global slot, and each owner waits
     until its device-side totals have reached the sums ("the expected number of
     incoming and outgoing data transfers")."""
-    mine = ctx.global_fence_begin()
-    everyone = _all_gather(mine.tobytes(), group)
+    mine, deferred = ctx.global_fence_begin(defer_error=True)
+    everyone = _all_gather(mine.tobytes(), group)                 # (a rank with a rejected batch still takes part)
     ctx.global_fence_end(np.frombuffer(b"".join(everyone), dtype=GLOBAL_COUNT_DTYPE), timeout_ms)
+    if deferred is not None:
+        raise deferred
 
 
 def exchange_in_process(ctxs, tag: int, contributions) -> list:
@@ -61,7 +63,10 @@ def exchange_in_process(ctxs, tag: int, contributions) -> list:
 
 
 def fence_in_process(ctxs, timeout_ms: int = 0) -> None:
-    lines = [c.global_fence_begin() for c in ctxs]
-    everyone = np.concatenate(lines) if lines else np.zeros(0, dtype=GLOBAL_COUNT_DTYPE)
+    got = [c.global_fence_begin(defer_error=True) for c in ctxs]
+    everyone = np.concatenate([g[0] for g in got]) if got else np.zeros(0, dtype=GLOBAL_COUNT_DTYPE)
     for c in ctxs:
         c.global_fence_end(everyone, timeout_ms)
+    for _, deferred in got:
+        if deferred is not None:
+            raise deferred

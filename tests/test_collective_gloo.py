@@ -28,14 +28,15 @@ class Stub:
     def global_exchange(self, tag, handles):
         self.handles = list(handles)
         return [1000 + i for i in range(len(handles))]
-    def global_fence_begin(self):
+    def global_fence_begin(self, defer_error=False):
         a = np.zeros(rank + 1, dtype=GLOBAL_COUNT_DTYPE)
         a["tag"], a["key"], a["sent"], a["recv"] = 3, np.arange(rank + 1), 10 * rank, rank
-        return a
+        return (a, RuntimeError("rejected batch") if rank == 1 and self.fail else None) if defer_error else a
     def global_fence_end(self, counts, timeout_ms=0):
         self.counts = np.array(counts)
 
 s = Stub()
+s.fail = False
 contrib = [(10 * rank + j, 5 + j) for j in range(rank + 1)]          # rank 0 volunteers 1 slot, rank 1 two
 out = collective.exchange_global_slots(s, 3, contrib)
 expect = [(r, 10 * r + j, 5 + j) for r in range(world) for j in range(r + 1)]
@@ -44,6 +45,14 @@ assert out == {k: 1000 + i for i, (_, k, _) in enumerate(expect)}, out
 collective.fence_global(s)
 assert len(s.counts) == sum(r + 1 for r in range(world))
 assert sorted(s.counts["sent"].tolist()) == sorted(10 * r for r in range(world) for _ in range(r + 1))
+# a rank whose epoch holds a rejected batch still completes the exchange with its peers, then raises
+s.fail, s.counts = True, None
+try:
+    collective.fence_global(s)
+    raised = False
+except RuntimeError:
+    raised = True
+assert raised == (rank == 1) and len(s.counts) == sum(r + 1 for r in range(world))
 empty = collective.exchange_global_slots(s, 4, [] if rank == 0 else [(1, 2)])    # "zero or more"
 assert list(empty) == [1]
 dist.destroy_process_group()

@@ -210,6 +210,40 @@ def test_golden_put_get_self_zero_oob_on_gpu(hicr, golden_dir):
         _close(ctxs)
 
 
+def test_rejected_batch_does_not_break_the_global_fence(hicr):
+    """Instance 0's device table holds a put past the end of the peer's slot: the batch has no effect
+    and the error surfaces at instance 0's half of the global fence -- after the count exchange, so
+    instance 1's own put is fenced and counted as usual (oracle: same statuses, bytes and counts)."""
+    world = World(2)
+    mem = [[np.full(64, 1 + i, np.uint8), np.zeros(64, np.uint8)] for i in range(2)]
+    oid = [[world.inst[i].slot_register(a) for a in mem[i]] for i in range(2)]
+    rc, og = world.exchange(5, [[(0, oid[0][1])], [(1, oid[1][1])]])
+    ctxs = _instances(hicr, 2)
+    try:
+        bufs = [[torch.from_numpy(a.copy()).cuda() for a in mem[i]] for i in range(2)]
+        gid = [[ctxs[i].slot_register(t) for t in bufs[i]] for i in range(2)]
+        gg = hicr.collective.exchange_in_process(ctxs, 5, [[(0, gid[0][1])], [(1, gid[1][1])]])
+        bad = np.concatenate([_one(gg[0][1], 0, gid[0][0], 0, 16), _one(gg[0][1], 60, gid[0][0], 0, 16)])
+        good = _one(gg[1][0], 8, gid[1][0], 0, 32)
+        assert world.inst[0].memcpy_batch(bad) == (oracle.ERR_OUT_OF_BOUNDS, 1)
+        assert world.inst[1].memcpy_batch(good)[0] == oracle.OK
+        world.fence_all()
+        t = torch.from_numpy(bad.view(np.uint8).copy()).cuda()
+        ctxs[0].memcpy_batch(t, n=2)
+        ctxs[1].memcpy_batch(good)
+        with pytest.raises(hicr.HicrError) as e:
+            hicr.collective.fence_in_process(ctxs)
+        assert (e.value.status, e.value.first_bad) == (hicr.HICR_ERR_OUT_OF_BOUNDS, 1)
+        for i in range(2):
+            for a, tt in zip(mem[i], bufs[i]):
+                assert tt.cpu().numpy().tobytes() == a.tobytes()
+            for s_ in list(gid[i]) + list(gg[i].values()):
+                assert ctxs[i].slot_counters(s_) == world.inst[i].slot_counters(s_)
+            assert ctxs[i].global_counters(gid[i][1]) == world.inst[i].slot_global_counters(oid[i][1])
+    finally:
+        _close(ctxs)
+
+
 def _compare_with_oracle(hicr, w, ctxs, bufs, ids, gg):
     world, mem, oids, og = oracle_run(w)
     assert ids == oids and gg == og
