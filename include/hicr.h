@@ -5,8 +5,10 @@
  * model (arxiv 2509.01425, cited below as PAPER.md:<line>), i.e. the Communication
  * Manager's `memcpy` between registered Local Memory Slots, completed by `fence`
  * (listing PAPER.md:524-535), plus the Channels frontend's
- * fixed-size-token circular buffer.  One GPU, one memory space
- * (that GPU's HBM).  Every step of the path runs in hand-written sm_100a CUDA kernels;
+ * fixed-size-token circular buffer, plus Global Memory Slots: slots
+ * exchanged between instances and reached by put / get.  One context =
+ * one GPU's HBM as its memory space; other instances' slots are reached over CUDA IPC peer
+ * mappings.  Every step of the path runs in hand-written sm_100a CUDA kernels;
  * there is no CPU fallback: without a CUDA device every call returns HICR_ERR_CUDA.
  *
  * Conventions
