@@ -117,16 +117,19 @@ import pynvml as nv
 nv.nvmlInit()
 h = nv.nvmlDeviceGetHandleByIndex(int(sys.argv[1]))
 period = float(sys.argv[2])
-print("max %d" % nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM), flush=True)
-while True:
+def reasons():
     try:
-        r = int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
+        return int(nv.nvmlDeviceGetCurrentClocksEventReasons(h))
     except Exception:
         try:
-            r = int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
+            return int(nv.nvmlDeviceGetCurrentClocksThrottleReasons(h))
         except Exception:
-            r = 0
-    print("%.6f %d %d" % (time.time(), nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM), r), flush=True)
+            return 0
+for _ in range(3):                      # the first queries of a process take milliseconds: have them behind us
+    reasons(); nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM)
+print("max %d" % nv.nvmlDeviceGetMaxClockInfo(h, nv.NVML_CLOCK_SM), flush=True)
+while True:
+    print("%.6f %d %d" % (time.time(), nv.nvmlDeviceGetClockInfo(h, nv.NVML_CLOCK_SM), reasons()), flush=True)
     time.sleep(period)
 """
 
@@ -426,9 +429,9 @@ def run_cuda(args):
                     ctx.fence()
 
         # ---- device-resident arm (value): K steps, nothing else on the stream
+        clocks = ClockSampler(local)     # (its process is up and sampling before the warm-up is over)
         run_steps(Wm)
         ctx.fence()
-        clocks = ClockSampler(local)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         l0 = ctx.launch_count()
