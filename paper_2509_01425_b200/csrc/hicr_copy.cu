@@ -224,6 +224,21 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     uint4 alo = make_uint4(0, 0, 0, 0), ahi = alo;
     const uint64_t tile0 = (uint64_t)blockIdx.x * kThreads;
     if (tile0 + tid < a.n) load_desc_raw(a.descs + tile0 + tid, alo, ahi);
+    // ---- warp tickets of phase B2.  The first ticket of every warp is static (warp g owns
+    // descriptors [g c0, (g+1) c0)); the others are atomics on a shared cursor that counts
+    // from the end of the static tickets.
+    const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
+    const unsigned gdiv = kGss * nw;
+    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, 1u), kMaxGroup); };
+    // (a multiple of 8 when it can be: team-sized descriptors are copied 8 at a time)
+    const unsigned cnt_static0 = ticket_size(n, 0), cnt_static = cnt_static0 >= 8 ? cnt_static0 & ~7u : cnt_static0;
+    const unsigned static_end = nw * cnt_static;
+    // ... and so are the descriptors of this warp's static first ticket: their round trip (cold: another
+    // CTA's tile) hides behind phase A instead of sitting between it and the arrival at the barrier
+    const unsigned first0_early = (blockIdx.x * kWarps + warp) * cnt_static;
+    uint4 flo = make_uint4(0, 0, 0, 0), fhi = flo;
+    const bool fhave = (unsigned)lane < cnt_static && first0_early + lane < n;
+    if (fhave) load_desc_raw(a.descs + first0_early + lane, flo, fhi);
     if (n_slots <= kSlotCache)
         for (uint32_t i = tid; i < n_slots; i += kThreads) {
             const uint4 v = __ldg(reinterpret_cast<const uint4 *>(a.slots + i));
@@ -245,15 +260,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
 
-    // ---- warp tickets of phase B2.  The first ticket of every warp is static (warp g owns
-    // descriptors [g c0, (g+1) c0)); the others are atomics on a shared cursor that counts
-    // from the end of the static tickets.
-    const unsigned n = (unsigned)a.n, nw = gridDim.x * kWarps;
-    const unsigned gdiv = kGss * nw;
-    auto ticket_size = [&](unsigned total, unsigned seen) { return min(max((total - min(seen, total)) / gdiv, 1u), kMaxGroup); };
-    // (a multiple of 8 when it can be: team-sized descriptors are copied 8 at a time)
-    const unsigned cnt_static0 = ticket_size(n, 0), cnt_static = cnt_static0 >= 8 ? cnt_static0 & ~7u : cnt_static0;
-    const unsigned static_end = nw * cnt_static;
     __syncthreads();
 
     // ================================================================ phase A (a2, a3, a6)
@@ -346,9 +352,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0;
     unsigned cnt1 = a.hand_out != kHandOutStatic ? ticket_size(n, static_end) : 0u, base1 = 0;
     if (tid == 0 && a.hand_out != kHandOutStatic) base1 = atomicAdd(&ctl->next_desc, cnt1 * kWarps);
-    uint4 flo = make_uint4(0, 0, 0, 0), fhi = flo;
-    const bool fhave = (unsigned)lane < cnt_static && first0 + lane < n;
-    if (fhave) load_desc_raw(a.descs + first0 + lane, flo, fhi);
 
     // ================================================================ grid barrier
     uint64_t src = 0, dst = 0;
