@@ -258,6 +258,25 @@ def test_stream_from_a_ring_in_use(hicr, T, C, pre, batches):
         p.close()
 
 
+@pytest.mark.parametrize("cluster", ["0", "1"])
+def test_pipeline_with_and_without_clusters(hicr, monkeypatch, cluster):
+    """HICR_PIPE_CLUSTER (read per call): the device-resident runs with the two ends of a ring as one
+    thread-block cluster (default) and as two CTAs of a cooperative launch (the path for devices or
+    shapes without clusters) -- the same results as the oracle either way."""
+    monkeypatch.setenv("HICR_PIPE_CLUSTER", cluster)
+    _mpsc_both(hicr, W.mpsc(producers=148, n_tokens=6000, token_bytes=64, capacity=1024, max_batch=256), 256)
+    _mpsc_both(hicr, W.mpsc(producers=3, n_tokens=2000, token_bytes=48, capacity=64, max_batch=20), 20)
+    T, C, N = 256, 1024, 100000
+    w = W.spsc(n_tokens=N, token_bytes=T, capacity=C, max_batch=1024)
+    p = Pair(hicr, T, C, w.source_image(0), N * T)
+    try:
+        _oracle_spsc(p, w)
+        p.ch.stream(p.ids[1], 0, p.ids[2], 0, w.batches[0])
+        p.check("spsc, HICR_PIPE_CLUSTER=" + cluster)
+    finally:
+        p.close()
+
+
 def _mpsc_both(hicr, w, max_batch):
     T, C, P, N = w.token_bytes, w.capacity, w.producers, w.n_tokens
     # oracle: P independent SPSC channels driven in the seeded interleaving
