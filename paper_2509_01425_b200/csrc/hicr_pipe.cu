@@ -138,6 +138,7 @@ struct PipeArgs {
     uint32_t piece_shift;                // tokens per piece = 1 << piece_shift
     uint32_t stage_bytes;
     uint32_t workers;
+    uint32_t ends;                       // CTAs per end (cluster kernel: a cluster holds 2 * ends CTAs)
     unsigned long long T, C, tokens, max_batch, n_batches;
     const unsigned long long *batches;
     SlotCnt *cnt;
@@ -149,15 +150,20 @@ struct PipeArgs {
 // counters in L2; the counters in device memory follow with plain stores and are final at kernel end.
 template <bool CL>
 __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_smem, uint64_t *bars, unsigned long long *next_start,
-                                          unsigned long long *mirror)
+                                          unsigned long long *mirror, unsigned long long *peer_min)
 {
     const int lane = threadIdx.x & 31;
     const unsigned warp = threadIdx.x >> 5, W = a.workers;
-    const bool producer = CL ? cluster_ctarank() == 0 : blockIdx.x < a.P;
-    const PipeRing r = a.rings[CL ? blockIdx.x / 2 : producer ? blockIdx.x : blockIdx.x - a.P];
+    // cluster: ranks 0 .. E-1 are the producer end's CTAs, E .. 2E-1 the consumer end's; CTA `e` of an end
+    // moves the pieces of its workers; the end's CTA 0 is its LEAD (it publishes the end's counter)
+    const unsigned E = CL ? a.ends : 1u, crank = CL ? cluster_ctarank() : 0u;
+    const bool producer = CL ? crank < E : blockIdx.x < a.P;
+    const unsigned e = CL ? crank % E : 0u;
+    const PipeRing r = a.rings[CL ? blockIdx.x / (2 * E) : producer ? blockIdx.x : blockIdx.x - a.P];
     const unsigned long long T = a.T, C = a.C, run_end = r.count0 + a.tokens;
     ChannelState *st = r.st;
     if (threadIdx.x < 32) next_start[threadIdx.x] = threadIdx.x < W ? r.count0 : ~0ull;
+    if (threadIdx.x < 8) peer_min[threadIdx.x] = threadIdx.x < E ? r.count0 : ~0ull;
     if (threadIdx.x == 0) *mirror = r.count0;
     if (lane == 0 && warp < W) {
         for (int s = 0; s < kPipeStages; s++) mbar_init(&bars[warp * kPipeStages + s], 1);
@@ -171,35 +177,52 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
         // first unfinished piece starts.  A worker's bulk writes are complete before it moves its value
         // (release / acquire at CTA scope), and the store below is a release at device scope.
         unsigned long long *counter = producer ? &st->head : &st->tail;
-        unsigned long long published = r.count0;
+        unsigned long long published = r.count0, fenced = r.count0;
+        const bool lead = e == 0;
         while (published < run_end) {
             unsigned long long v = ld_acquire_cta_shared_u64(&next_start[lane]);
 #pragma unroll
             for (int d = 16; d; d >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, d));
-            v = min(v, run_end);
+            v = min(v, run_end);          // this CTA's own frontier
+            if (CL && producer && v > fenced) {
+                // this SM's payload up to v is performed device-wide before anybody hears of it (every CTA of
+                // the end fences its own bulk writes; without the fence the consumers read stale ring bytes --
+                // measured, 148 rings)
+                if (lane == 0) __threadfence();
+                fenced = v;
+            }
+            if (CL && E > 1) {
+                if (!lead) {
+                    // report to the lead of this end (its peer_min[e])
+                    if (v > published && lane == 0) st_remote_shared_u64(&peer_min[e], producer ? 0u : E, v);
+                    published = max(published, v);
+                    continue;
+                }
+                unsigned long long pv = lane > 0 && lane < (int)E ? *reinterpret_cast<volatile unsigned long long *>(&peer_min[lane]) : ~0ull;
+#pragma unroll
+                for (int d = 4; d; d >>= 1) pv = min(pv, __shfl_xor_sync(0xffffffffu, pv, d));
+                v = min(v, __shfl_sync(0xffffffffu, pv, 0));   // the end's frontier: the minimum over its CTAs
+            }
             if (v > published) {
                 if (lane == 0) {
-                    // head: a release (payload first, then the counter; without the fence in it the consumers
-                    // read stale ring bytes -- measured, 148 rings).  tail: the ring reads behind it have
-                    // returned their data (the workers waited on their mbarriers), so a plain store cannot
-                    // let the producer overwrite anything still to be read; 8 % faster than a second release.
+                    // tail: the ring reads behind it have returned their data (the workers waited on their
+                    // mbarriers), so plain stores cannot let the producer overwrite anything still to be read
                     if (CL) {
-                        if (producer) __threadfence();   // the payload is performed device-wide before the other CTA hears of it
-                        st_remote_shared_u64(mirror, producer ? 1u : 0u, v);
+                        for (unsigned t = 0; t < E; t++) st_remote_shared_u64(mirror, (producer ? E : 0u) + t, v);
                         *reinterpret_cast<volatile unsigned long long *>(counter) = v;
-                    } else if (producer) st_release(counter, v);
-                    else *reinterpret_cast<volatile unsigned long long *>(counter) = v;
+                    } else if (producer) st_release(counter, v);   // payload first, then the counter (8 % faster
+                    else *reinterpret_cast<volatile unsigned long long *>(counter) = v;   // than a second release)
                 }
                 published = v;
             }
         }
-        if (!producer && lane == 0) {
+        if (!producer && e == 0 && lane == 0) {
             // the ring is through: one message per token on every slot it touched (reading 15)
             atomicAdd(&a.cnt[r.id_src].sent, a.tokens);
             atomicAdd(&a.cnt[r.id_ring].recv, a.tokens);
             atomicAdd(&a.cnt[r.id_ring].sent, a.tokens);
             atomicAdd(&a.cnt[r.id_dst].recv, a.tokens);
-            if (a.res && blockIdx.x == (CL ? 1u : a.P)) {
+            if (a.res && blockIdx.x == (CL ? E : a.P)) {
                 a.res->k = a.tokens;
                 a.res->head = CL ? run_end : ld_acquire(&st->head);
                 a.res->tail = published;
@@ -215,8 +238,8 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
     uint64_t *bar = &bars[warp * kPipeStages];
     PieceWalk wk;
     // the consumer pops what is there: one "push" of all the tokens, no push ends to respect
-    walk_init(wk, r.count0, a.tokens, warp, W, a.piece_shift, producer ? a.batches : nullptr, producer ? a.n_batches : 0,
-              producer ? a.max_batch : a.tokens);
+    walk_init(wk, r.count0, a.tokens, e * W + warp, E * W, a.piece_shift, producer ? a.batches : nullptr,
+              producer ? a.n_batches : 0, producer ? a.max_batch : a.tokens);
     const unsigned long long bias = r.count0;     // token a comes from / goes to (a - count0) * T of the source / sink
     unsigned k = 0;   // own pieces so far: stage k % 2, mbarrier parity (k / 2) & 1
 
@@ -289,8 +312,8 @@ __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_kernel(con
     extern __shared__ __align__(128) unsigned char dyn_smem[];   // [worker][stage][stage_bytes]
     __shared__ uint64_t bars[kPipeMaxWorkers * kPipeStages];
     __shared__ unsigned long long next_start[32];                // per worker: first token of its first unfinished piece
-    __shared__ unsigned long long mirror;
-    pipe_body<false>(a, dyn_smem, bars, next_start, &mirror);
+    __shared__ unsigned long long mirror, peer_min[8];
+    pipe_body<false>(a, dyn_smem, bars, next_start, &mirror, peer_min);
 }
 
 __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_cluster_kernel(const PipeArgs a)
@@ -298,8 +321,9 @@ __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_cluster_ke
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     __shared__ uint64_t bars[kPipeMaxWorkers * kPipeStages];
     __shared__ unsigned long long next_start[32];
-    __shared__ unsigned long long mirror;                        // the other end's counter, written by the other CTA
-    pipe_body<true>(a, dyn_smem, bars, next_start, &mirror);
+    __shared__ unsigned long long mirror;                        // the other end's counter, written by its lead CTA
+    __shared__ unsigned long long peer_min[8];                   // lead: the frontiers the end's other CTAs report
+    pipe_body<true>(a, dyn_smem, bars, next_start, &mirror, peer_min);
     cluster_sync_all();   // neither CTA leaves while the other may still write its mirror
 }
 
@@ -368,6 +392,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
     a.piece_shift = sh.piece_shift;
     a.stage_bytes = sh.stage_bytes;
     a.workers = sh.workers;
+    a.ends = 1;
     a.T = T;
     a.C = C;
     a.tokens = tokens;
@@ -385,14 +410,20 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
     // HICR_PIPE_CLUSTER=0 forces the cooperative path (the tests run both; read per call)
     const char *knob = getenv("HICR_PIPE_CLUSTER");
     if (!(knob && knob[0] == '0')) {
+        // CTAs per end.  One SM moves about 93 GB/s through its L2 port, i.e. 48 GB/s of payload in and out:
+        // a single ring gets two CTAs per end (config 5a: the lap of its 256 KiB ring then binds, 50.8 GB/s),
+        // four when the ring is large enough not to (1 MiB: 96 GB/s with two, 156-188 GB/s with four);
+        // many rings get one CTA per end and fill the device that way.
+        const unsigned E = P > 1 ? 1u : C * T >= (1u << 20) ? 4u : 2u;
+        a.ends = E;
         cudaLaunchConfig_t cfg = {};
-        cfg.gridDim = dim3(2 * P);
+        cfg.gridDim = dim3(2 * E * P);
         cfg.blockDim = dim3(32 * (sh.workers + 1));
         cfg.dynamicSmemBytes = sh.smem;
         cfg.stream = ctx->stream;
         cudaLaunchAttribute at[1];
         at[0].id = cudaLaunchAttributeClusterDimension;
-        at[0].val.clusterDim.x = 2;
+        at[0].val.clusterDim.x = 2 * E;
         at[0].val.clusterDim.y = 1;
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
@@ -404,7 +435,10 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
             e = cudaLaunchKernelExC(&cfg, (const void *)pipe_cluster_kernel, args);
             clustered = e == cudaSuccess;
         }
-        if (!clustered) (void)cudaGetLastError();
+        if (!clustered) {
+            (void)cudaGetLastError();
+            a.ends = 1;
+        }
     }
     if (!clustered)
     HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)pipe_kernel, dim3(2 * P), dim3(32 * (sh.workers + 1)), args,

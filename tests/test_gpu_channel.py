@@ -225,6 +225,7 @@ def test_spsc_stream_equals_call_sequence(hicr, T, C, N, maxb):
     (64, 48, 5, [100, 1, 1, 48, 49, 7]),                        # capacity not a power of two: pieces of 16 tokens
     (4096, 8, 3, [1, 30, 2, 9]),                                # two tokens per piece
     (16384, 4, 1, [5, 11]),                                     # a token larger than the default stage
+    (1024, 1024, 77, [3000, 1, 2048, 700]),                     # a 1 MiB ring: four CTAs per end
     (32, 1024, 9, [4000, 96]),                                  # 1 KiB pieces: the smallest the pipeline takes
     (16, 64, 2, [500]),                                         # pieces below 1 KiB: the vector kernels
 ])
