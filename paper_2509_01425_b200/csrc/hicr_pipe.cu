@@ -139,23 +139,32 @@ struct PipeArgs {
     uint32_t stage_bytes;
     uint32_t workers;
     uint32_t ends;                       // CTAs per end (cluster kernel: a cluster holds 2 * ends CTAs)
+    uint32_t fence_in_worker;            // cluster kernel: the producer's workers fence their own pieces
     unsigned long long T, C, tokens, max_batch, n_batches;
     const unsigned long long *batches;
     SlotCnt *cnt;
     CallResult *res;                     // ring 0's head / tail at the end of the run (hicr_channel_stream)
 };
 
+// The other end's counter as this CTA knows it: the minimum of what the other end's CTAs have written here.
+__device__ __forceinline__ unsigned long long mirror_min(const unsigned long long *mirror, unsigned E)
+{
+    unsigned long long v = *reinterpret_cast<const volatile unsigned long long *>(mirror);
+    for (unsigned t = 1; t < E; t++) v = min(v, *reinterpret_cast<const volatile unsigned long long *>(mirror + t));
+    return v;
+}
+
 // CL: the two ends of a ring are the two CTAs of a thread-block cluster and tell each other head / tail
 // through distributed shared memory (`mirror` of the other CTA) instead of through polls of the
 // counters in L2; the counters in device memory follow with plain stores and are final at kernel end.
 template <bool CL>
 __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_smem, uint64_t *bars, unsigned long long *next_start,
-                                          unsigned long long *mirror, unsigned long long *peer_min)
+                                          unsigned long long *mirror)
 {
     const int lane = threadIdx.x & 31;
     const unsigned warp = threadIdx.x >> 5, W = a.workers;
     // cluster: ranks 0 .. E-1 are the producer end's CTAs, E .. 2E-1 the consumer end's; CTA `e` of an end
-    // moves the pieces of its workers; the end's CTA 0 is its LEAD (it publishes the end's counter)
+    // moves the pieces of its own workers
     const unsigned E = CL ? a.ends : 1u, crank = CL ? cluster_ctarank() : 0u;
     const bool producer = CL ? crank < E : blockIdx.x < a.P;
     const unsigned e = CL ? crank % E : 0u;
@@ -163,8 +172,7 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
     const unsigned long long T = a.T, C = a.C, run_end = r.count0 + a.tokens;
     ChannelState *st = r.st;
     if (threadIdx.x < 32) next_start[threadIdx.x] = threadIdx.x < W ? r.count0 : ~0ull;
-    if (threadIdx.x < 8) peer_min[threadIdx.x] = threadIdx.x < E ? r.count0 : ~0ull;
-    if (threadIdx.x == 0) *mirror = r.count0;
+    if (threadIdx.x < 8) mirror[threadIdx.x] = threadIdx.x < E ? r.count0 : ~0ull;
     if (lane == 0 && warp < W) {
         for (int s = 0; s < kPipeStages; s++) mbar_init(&bars[warp * kPipeStages + s], 1);
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -177,45 +185,32 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
         // first unfinished piece starts.  A worker's bulk writes are complete before it moves its value
         // (release / acquire at CTA scope), and the store below is a release at device scope.
         unsigned long long *counter = producer ? &st->head : &st->tail;
-        unsigned long long published = r.count0, fenced = r.count0;
-        const bool lead = e == 0;
+        unsigned long long published = r.count0;
         while (published < run_end) {
             unsigned long long v = ld_acquire_cta_shared_u64(&next_start[lane]);
 #pragma unroll
             for (int d = 16; d; d >>= 1) v = min(v, __shfl_xor_sync(0xffffffffu, v, d));
-            v = min(v, run_end);          // this CTA's own frontier
-            if (CL && producer && v > fenced) {
-                // this SM's payload up to v is performed device-wide before anybody hears of it (every CTA of
-                // the end fences its own bulk writes; without the fence the consumers read stale ring bytes --
-                // measured, 148 rings)
-                if (lane == 0) __threadfence();
-                fenced = v;
-            }
-            if (CL && E > 1) {
-                if (!lead) {
-                    // report to the lead of this end (its peer_min[e])
-                    if (v > published && lane == 0) st_remote_shared_u64(&peer_min[e], producer ? 0u : E, v);
-                    published = max(published, v);
-                    continue;
-                }
-                unsigned long long pv = lane > 0 && lane < (int)E ? *reinterpret_cast<volatile unsigned long long *>(&peer_min[lane]) : ~0ull;
-#pragma unroll
-                for (int d = 4; d; d >>= 1) pv = min(pv, __shfl_xor_sync(0xffffffffu, pv, d));
-                v = min(v, __shfl_sync(0xffffffffu, pv, 0));   // the end's frontier: the minimum over its CTAs
-            }
+            v = min(v, run_end);          // this CTA's frontier
             if (v > published) {
                 if (lane == 0) {
-                    // tail: the ring reads behind it have returned their data (the workers waited on their
-                    // mbarriers), so plain stores cannot let the producer overwrite anything still to be read
+                    // head: payload first, then the counter -- a device-scope fence between them (without it the
+                    // consumers read stale ring bytes: measured, 148 rings).  tail: the ring reads behind it have
+                    // returned their data (the workers waited on their mbarriers), so plain stores cannot let the
+                    // producer overwrite anything still to be read (a second release measured 8 % slower).
                     if (CL) {
-                        for (unsigned t = 0; t < E; t++) st_remote_shared_u64(mirror, (producer ? E : 0u) + t, v);
-                        *reinterpret_cast<volatile unsigned long long *>(counter) = v;
-                    } else if (producer) st_release(counter, v);   // payload first, then the counter (8 % faster
-                    else *reinterpret_cast<volatile unsigned long long *>(counter) = v;   // than a second release)
+                        // every CTA of an end fences its own SM's writes and tells EVERY CTA of the other end its
+                        // own frontier (slot e of their `mirror`); they take the minimum themselves
+                        if (producer && !a.fence_in_worker) __threadfence();
+                        for (unsigned t = 0; t < E; t++) st_remote_shared_u64(&mirror[e], (producer ? E : 0u) + t, v);
+                        if (E == 1) *reinterpret_cast<volatile unsigned long long *>(counter) = v;
+                    } else if (producer) st_release(counter, v);
+                    else *reinterpret_cast<volatile unsigned long long *>(counter) = v;
                 }
                 published = v;
             }
         }
+        // (several CTAs per end: the counter in device memory gets the end's final value; nobody reads it before)
+        if (CL && E > 1 && e == 0 && lane == 0) *reinterpret_cast<volatile unsigned long long *>(counter) = run_end;
         if (!producer && e == 0 && lane == 0) {
             // the ring is through: one message per token on every slot it touched (reading 15)
             atomicAdd(&a.cnt[r.id_src].sent, a.tokens);
@@ -265,11 +260,15 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
             // room: every position of the piece has been popped ("as long as the buffer has not filled up")
             const unsigned long long end_abs = cur.a + cur.len;
             while (tail_seen + C < end_abs)
-                tail_seen = CL ? *reinterpret_cast<volatile unsigned long long *>(mirror) : ld_acquire(&st->tail);
+                tail_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->tail);
             mbar_wait(bar + s, (k / kPipeStages) & 1);
             bulk_s2g(r.ring + (cur.a % C) * T, stage + (size_t)s * a.stage_bytes, (unsigned)(cur.len * T));
             bulk_commit();
             bulk_wait_all();       // the payload is written (complete, not just read out of shared memory)
+            // (where the ring's lap binds -- a single small ring -- the fence head needs is taken here, by every
+            // worker for its own piece in parallel, instead of by the committer for all: config 5a 70.6 -> 67.2 ms;
+            // where the workers bind -- a large ring -- that costs a quarter of the throughput)
+            if (CL && a.fence_in_worker) __threadfence();
             st_release_cta_shared_u64(&next_start[warp], have_next ? nxt.a : ~0ull);   // the committer takes it from here
             cur = nxt;
             have = have_next;
@@ -287,7 +286,7 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
         const unsigned s = k % kPipeStages;
         const unsigned long long end_abs = cur.a + cur.len;
         while (head_seen < end_abs)
-            head_seen = CL ? *reinterpret_cast<volatile unsigned long long *>(mirror) : ld_acquire(&st->head);
+            head_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->head);
         if (k >= kPipeStages) bulk_wait_read<kPipeStages - 1>();   // the sink store that last read this stage
         const unsigned bytes = (unsigned)(cur.len * T);
         mbar_expect_tx(bar + s, bytes);
@@ -312,8 +311,8 @@ __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_kernel(con
     extern __shared__ __align__(128) unsigned char dyn_smem[];   // [worker][stage][stage_bytes]
     __shared__ uint64_t bars[kPipeMaxWorkers * kPipeStages];
     __shared__ unsigned long long next_start[32];                // per worker: first token of its first unfinished piece
-    __shared__ unsigned long long mirror, peer_min[8];
-    pipe_body<false>(a, dyn_smem, bars, next_start, &mirror, peer_min);
+    __shared__ unsigned long long mirror[8];
+    pipe_body<false>(a, dyn_smem, bars, next_start, mirror);
 }
 
 __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_cluster_kernel(const PipeArgs a)
@@ -321,9 +320,8 @@ __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_cluster_ke
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     __shared__ uint64_t bars[kPipeMaxWorkers * kPipeStages];
     __shared__ unsigned long long next_start[32];
-    __shared__ unsigned long long mirror;                        // the other end's counter, written by its lead CTA
-    __shared__ unsigned long long peer_min[8];                   // lead: the frontiers the end's other CTAs report
-    pipe_body<true>(a, dyn_smem, bars, next_start, &mirror, peer_min);
+    __shared__ unsigned long long mirror[8];                     // slot e: the frontier of CTA e of the other end, written by it
+    pipe_body<true>(a, dyn_smem, bars, next_start, mirror);
     cluster_sync_all();   // neither CTA leaves while the other may still write its mirror
 }
 
@@ -393,6 +391,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
     a.stage_bytes = sh.stage_bytes;
     a.workers = sh.workers;
     a.ends = 1;
+    a.fence_in_worker = 0;
     a.T = T;
     a.C = C;
     a.tokens = tokens;
@@ -416,6 +415,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
         // many rings get one CTA per end and fill the device that way.
         const unsigned E = P > 1 ? 1u : C * T >= (1u << 20) ? 4u : 2u;
         a.ends = E;
+        a.fence_in_worker = E == 2;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(2 * E * P);
         cfg.blockDim = dim3(32 * (sh.workers + 1));
@@ -438,6 +438,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
         if (!clustered) {
             (void)cudaGetLastError();
             a.ends = 1;
+            a.fence_in_worker = 0;
         }
     }
     if (!clustered)
