@@ -846,7 +846,7 @@ def run_channel(args):
                      "achieved": gbs / 2, "peak": peak, "unit": UNIT, "frac": gbs / 2 / peak, "traffic": None,
                      "peak_source": peak_src,
                      "note": "DRAM sees source and sink only (the ring lives in L2): algorithmic DRAM bytes = 2 x payload; "
-                             "the bound that binds is one producer CTA and one consumer CTA per ring, not HBM"},
+                             "what binds is the lap of a ring (write -> publish -> read -> publish), see profiles/r02_channels.md"},
         "cpu_baseline": None if args.no_cpu_baseline else oracle_channel_sample(w, args.cpu_seconds),
         "clocks": clk, "sink_equals_source": bool(ok),
     }

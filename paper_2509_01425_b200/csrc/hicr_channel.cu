@@ -325,8 +325,8 @@ mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, u
             ring_copy<2, true>(ring, ring_bytes, (start % C) * T, src + pushed * T, k * T, tid, kMpscThreads);
             __syncthreads();
             if (tid == 0) {
-                unsigned ns = 20;
-                while (ld_acquire(&st->head) != start) backoff(ns);   // commit in reservation order
+                while (ld_acquire(&st->head) != start) {}   // commit in reservation order (the wait is on the critical path
+                                                            // of the ring's lap: no back-off)
                 st_release(&st->head, start + k);
             }
             pushed += k;
@@ -350,7 +350,9 @@ mpsc_locking_kernel(ChannelState *st, unsigned long long *reserve, uint32_t P, u
         const uint64_t k = sh_k;
         ring_copy<4, false>(ring, ring_bytes, (tail % C) * T, dst + popped * T, k * T, tid, kMpscThreads);
         __syncthreads();
-        if (tid == 0) st_release(&st->tail, tail + k);
+        // (every thread's ring loads have returned -- their values went into the stores before the barrier -- so a
+        // plain store frees the positions; a release would also wait for the sink stores to drain)
+        if (tid == 0) *reinterpret_cast<volatile unsigned long long *>(&st->tail) = tail + k;
         tail += k;
         popped += k;
     }
