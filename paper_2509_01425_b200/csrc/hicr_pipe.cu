@@ -340,12 +340,13 @@ static bool pipe_shape(hicr_ctx *ctx, uint32_t P, uint64_t T, uint64_t C, PipeSh
     const unsigned per_sm = (2 * P + ctx->num_sms - 1) / ctx->num_sms;     // CTAs that must share an SM
     // shared memory of an SM, less what the system keeps per CTA and the static part
     const size_t budget = std::min<size_t>((size_t)max_smem, (size_t)(228 * 1024) / per_sm - 2048);
-    // One ring: 12 workers x 2 x 8 KiB (the ring round trip binds; more bytes in flight measured the same).
-    // Many rings: 3 workers x 2 x 16 KiB per end (5.2 ms for 148 rings against 5.5 ms with 6 x 8 KiB).
-    unsigned stage = P == 1 ? 8192 : 16384;
+    // Per CTA: 6 workers x 2 stages x 16 KiB for one ring (config 5a: 63.7 ms against 67.3 with 12 x 8 KiB, 73.3
+    // with 24 x 4 KiB), 3 x 2 x 16 KiB for many rings, two CTAs per SM (148 rings: 4.23 ms against 4.33 with
+    // 6 x 8 KiB and 4.57 with 12 x 4 KiB): fewer, larger pieces mean fewer publications per lap.
+    unsigned stage = 16384;
     while (stage < T && (size_t)kPipeStages * 2 * stage <= budget) stage *= 2;
     while (stage > 1024 && budget < (size_t)kPipeStages * stage) stage /= 2;
-    unsigned workers = (unsigned)std::min<size_t>(budget / ((size_t)kPipeStages * stage), P == 1 ? 12 : 3);
+    unsigned workers = (unsigned)std::min<size_t>(budget / ((size_t)kPipeStages * stage), P == 1 ? 6 : 3);
     workers = std::min<unsigned>(workers, kPipeMaxWorkers);
     if (workers < 1) return false;
     // tokens per piece: the largest power of two that divides C and fits a stage (the wrap is then a cut too)
@@ -415,7 +416,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
         // many rings get one CTA per end and fill the device that way.
         const unsigned E = P > 1 ? 1u : C * T >= (1u << 20) ? 4u : 2u;
         a.ends = E;
-        a.fence_in_worker = E == 2;
+        a.fence_in_worker = E == 2 || P > 1;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3(2 * E * P);
         cfg.blockDim = dim3(32 * (sh.workers + 1));
