@@ -632,10 +632,10 @@ def run_cuda(args):
 # --------------------------------------------------------------------------- channel configs
 CHANNEL_TEXT = {
     "spsc_stream": "config 5a SPSC, device-resident run: 256 B tokens, capacity 1024, 2^24 tokens, batches U{1..1024}, "
-                   "producer CTA and consumer CTA in one kernel",
+                   "one kernel: a thread-block cluster with two producer CTAs and two consumer CTAs on the one ring",
     "spsc_calls": "config 5a SPSC, host-call path: push(b_i) then pop(max = capacity), one launch per call",
     "mpsc": "config 5b non-locking MPSC: 148 producers (one CTA per SM), 64 B tokens, 2^20 tokens each, rings of 1024, "
-            "single consumer CTA",
+            "one logical consumer = one consumer CTA per ring (producer and consumer of a ring form a thread-block cluster)",
     "mpsc_locking": "config 5b's shape in the paper's LOCKING mode (SURVEY.md S8(f) 2): 148 producers share ONE ring of 1024 "
                     "tokens of 64 B through atomic reservation and in-order commit, 2^20 tokens each, single consumer CTA",
 }
@@ -842,7 +842,7 @@ def run_channel(args):
                 "d2h_bytes_per_step": 32 * (2 * len(w.batches[0]) if name == "spsc_calls" else 1),
                 "ms_per_step": 1e3 * t_host / K, "what": "host wall clock around the blocking calls"},
         "gpu_launches": int(launches),
-        "roofline": {"bound": "hbm", "kernel": {"mpsc": "mpsc_stream_kernel", "mpsc_locking": "mpsc_locking_kernel"}.get(name, "spsc_stream_kernel"),
+        "roofline": {"bound": "hbm", "kernel": {"mpsc": "pipe_cluster_kernel", "spsc_stream": "pipe_cluster_kernel", "mpsc_locking": "mpsc_locking_kernel"}.get(name, "channel_call_kernel"),
                      "achieved": gbs / 2, "peak": peak, "unit": UNIT, "frac": gbs / 2 / peak, "traffic": None,
                      "peak_source": peak_src,
                      "note": "DRAM sees source and sink only (the ring lives in L2): algorithmic DRAM bytes = 2 x payload; "
