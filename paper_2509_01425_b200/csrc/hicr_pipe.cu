@@ -326,10 +326,14 @@ __global__ void __launch_bounds__((kPipeMaxWorkers + 1) * 32, 1) pipe_cluster_ke
 }
 
 // Shape of a run: workers per end, stage size, tokens per piece; false if the bulk-copy pipeline
-// cannot take it (alignment, pieces too small, co-residency of 2 P CTAs).
+// cannot take it (alignment, pieces too small).  coresident: all 2 P CTAs fit the device at once, which the
+// cooperative variant needs (its ends spin on each other across CTAs the hardware schedules one by one);
+// the cluster variant does not: a ring's two ends are one cluster, scheduled together, and rings are
+// independent, so any number of rings runs, a wave of clusters at a time.
 struct PipeShape {
     unsigned workers, stage_bytes, piece_shift;
     size_t smem;
+    bool coresident;
 };
 
 static bool pipe_shape(hicr_ctx *ctx, uint32_t P, uint64_t T, uint64_t C, PipeShape *out)
@@ -337,7 +341,8 @@ static bool pipe_shape(hicr_ctx *ctx, uint32_t P, uint64_t T, uint64_t C, PipeSh
     if (T % 16 != 0 || T == 0) return false;
     int max_smem = 0;
     if (cudaDeviceGetAttribute(&max_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, ctx->device) != cudaSuccess) return false;
-    const unsigned per_sm = (2 * P + ctx->num_sms - 1) / ctx->num_sms;     // CTAs that must share an SM
+    // CTAs that share an SM (at most two: beyond that the rings run in waves)
+    const unsigned per_sm = std::min<unsigned>(2u, (2 * P + ctx->num_sms - 1) / ctx->num_sms);
     // shared memory of an SM, less what the system keeps per CTA and the static part
     const size_t budget = std::min<size_t>((size_t)max_smem, (size_t)(228 * 1024) / per_sm - 2048);
     // Per CTA: 6 workers x 2 stages x 16 KiB for one ring (config 5a: 63.7 ms against 67.3 with 12 x 8 KiB, 73.3
@@ -368,7 +373,8 @@ static bool pipe_shape(hicr_ctx *ctx, uint32_t P, uint64_t T, uint64_t C, PipeSh
         (void)cudaGetLastError();
         return false;
     }
-    return (uint64_t)resident * ctx->num_sms >= 2ull * P;   // both ends of every ring spin on each other
+    out->coresident = (uint64_t)resident * ctx->num_sms >= 2ull * P;
+    return true;
 }
 
 // Runs the pipeline if the shape allows it (*ran = true) on the context's stream; the caller
@@ -442,6 +448,7 @@ int pipe_run(hicr_ctx *ctx, const PipeRing *h_rings, PipeRing *d_rings, uint32_t
             a.fence_in_worker = 0;
         }
     }
+    if (!clustered && !sh.coresident) return HICR_OK;   // too many rings for a cooperative launch: the caller's other path
     if (!clustered)
     HICR_CUDA(ctx, cudaLaunchCooperativeKernel((const void *)pipe_kernel, dim3(2 * P), dim3(32 * (sh.workers + 1)), args,
                                                sh.smem, ctx->stream));

@@ -321,7 +321,8 @@ def _mpsc_both(hicr, w, max_batch):
 
 
 @pytest.mark.parametrize("P,N,T,C,maxb", [(1, 5000, 64, 16, 16), (5, 3000, 8, 32, 48), (148, 20000, 64, 1024, 256),
-                                          (40, 1000, 100, 3, 7)])
+                                          (40, 1000, 100, 3, 7),
+                                          (700, 600, 64, 64, 40)])     # more rings than fit the device at once: waves of clusters
 def test_mpsc_stream(hicr, P, N, T, C, maxb):
     """Non-locking MPSC: one ring per producer, single consumer; per-producer
     sink = per-producer source, head_p = tail_p = N, independent of the interleaving."""
