@@ -811,7 +811,7 @@ extern "C" int hicr_memcpy_batch(hicr_ctx_t *ctx, const hicr_desc_t *descs, uint
         units = nc + (ns + kWarps - 1) / kWarps;
         ctx->used_stage.push_back(b);
         // pinned staging is device-accessible under unified addressing: short tables stay there
-        d_descs = static_cast<const hicr_desc_t *>(n <= kZeroCopyDescs ? b.host : b.dev);
+        d_descs = static_cast<const hicr_desc_t *>(table_read_in_place(descs, n) ? b.host : b.dev);
         // checked against the host mirror of the slot table, which the device copy follows in
         // stream order: with no chunk queue to wait for either, the kernel needs no barrier
         skip_barrier = nc == 0;

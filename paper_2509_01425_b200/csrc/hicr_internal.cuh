@@ -651,6 +651,7 @@ int drain_epoch(hicr_ctx *ctx, bool final_fence);
 int refresh_counters(hicr_ctx *ctx);
 int engine_setup(hicr_ctx *ctx);
 void launch_cache_free(hicr_ctx *ctx);
+bool table_read_in_place(const hicr_desc_t *descs, uint64_t n);
 int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const StageBlock &b, uint64_t *first_bad,
                 int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes);
 int bad_to_status(unsigned id);

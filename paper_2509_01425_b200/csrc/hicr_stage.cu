@@ -143,6 +143,23 @@ private:
     std::atomic<bool> stop_{false};
 };
 
+// Does the kernel read the staged table straight from pinned host memory (no copy to the device)?
+// Short tables: yes (32 KiB over PCIe costs less than enqueueing a copy).  Long tables: only when they
+// look like bulk pages -- 64 evenly spaced descriptors all between 2 KiB and kSmallMax bytes -- because
+// then the copy phase is long enough to hide the descriptor fetches over PCIe behind it and the 2 MiB
+// of config 2 need not cross the bus before the kernel may start (end to end 211 -> 185 us); small
+// descriptors (config 4: 149 -> 154 us) and tables with large ones (3a: 3.53 -> 3.64 ms) keep the copy.
+// A wrong guess costs time, never correctness: the kernel reads the same bytes either way.
+bool table_read_in_place(const hicr_desc_t *descs, uint64_t n)
+{
+    if (n <= kZeroCopyDescs) return true;
+    for (uint64_t k = 0; k < 64; k++) {
+        const uint64_t sz = descs[k * (n / 64)].size;
+        if (sz < 2048 || sz > kSmallMax) return false;
+    }
+    return true;
+}
+
 // (a2) for a host table: check + stage `descs` into the pinned block `b`, send it to b.dev on
 // the context's stream.  Returns HICR_OK or a CUDA failure; *bad_status = HICR_OK or the status of
 // the lowest bad index (*first_bad), with nothing to launch.  Totals: chunk-queue bound, small
@@ -151,6 +168,7 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
                 int *bad_status, uint64_t *n_chunk_bound, uint64_t *n_small, uint64_t *small_bytes)
 {
     constexpr uint64_t kPiece = 4096, kSendPieces = 4;
+    const bool in_place = table_read_in_place(descs, n);
     StageJob j;
     j.in = descs;
     j.out = static_cast<hicr_desc_t *>(b.host);
@@ -192,8 +210,8 @@ int stage_table(hicr_ctx *ctx, const hicr_desc_t *descs, uint64_t n, const Stage
             ready++;
         }
         if (rc != HICR_OK || *bad_status != HICR_OK) break;
-        if (n <= kZeroCopyDescs) {
-            sent = ready;   // short table: the kernel reads the pinned staging block in place (no copy to enqueue)
+        if (in_place) {
+            sent = ready;   // the kernel reads the pinned staging block in place (no copy to enqueue)
         } else if (ready - sent >= kSendPieces || (ready == j.n_pieces && ready > sent)) {
             const uint64_t i0 = sent * kPiece, i1 = std::min(n, ready * kPiece);
             cudaError_t e = cudaMemcpyAsync(static_cast<hicr_desc_t *>(b.dev) + i0, j.out + i0, (i1 - i0) * sizeof(hicr_desc_t),
