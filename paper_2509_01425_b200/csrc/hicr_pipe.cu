@@ -9,11 +9,14 @@
 // two ENDS, each one CTA, so the single LOGICAL consumer of the MPSC set is P CTAs, one per ring;
 // each ring's tail keeps a single writer and each producer's order is kept (per-producer FIFO).
 // Head and tail -- the 64-bit counters of ChannelState -- are all the two ends tell each other.
-// pipe_cluster_kernel: the two ends of ring r are the two CTAs of a thread-block cluster (rank 0
-// produces, rank 1 consumes); the hardware schedules them together, and each end writes its counter
-// into the other's shared memory (distributed shared memory) as well as to device memory, so the
-// other end's workers wait on a local word.  pipe_kernel (devices or shapes without clusters): CTA
-// r < P produces, CTA P + r consumes, cooperative launch, the ends poll the counters in L2.
+// pipe_cluster_kernel: the ends of ring r are the CTAs of ONE thread-block cluster -- E producer CTAs
+// (ranks 0 .. E-1) and E consumer CTAs (ranks E .. 2E-1); E = 1 for many rings, 2 or 4 for a single
+// ring (one SM moves 48 GB/s of payload in and out, no more).  The hardware schedules a cluster's
+// CTAs together, so the ends may spin on each other whatever else runs (rings are independent: any
+// number of rings runs, a wave of clusters at a time), and every CTA writes its progress into the
+// shared memory of every CTA of the other end (distributed shared memory), whose workers wait on
+// local words.  pipe_kernel (no clusters, or HICR_PIPE_CLUSTER=0): CTA r < P produces, CTA P + r
+// consumes, cooperative launch of 2 P co-resident CTAs, the ends poll the counters in L2.
 //
 // Inside an end the token stream is cut into PIECES -- at the ends of the pushes (the batch list
 // of hicr_channel_stream, or every max_batch tokens) and at every multiple of `piece_tokens`
@@ -26,14 +29,14 @@
 //             positions are then free); stage -> sink without waiting.
 // Each worker publishes, in shared memory, where its next unfinished piece starts.  Pieces tile
 // the stream and a worker finishes its own in order, so every token below the MINIMUM of those
-// W values is through: that minimum is the FRONTIER.  One more warp, the COMMITTER, keeps
-// taking the minimum (one value per lane, a warp shuffle reduction) and stores it to head (tail)
-// -- "payload first, then the counter", one writer per counter; head with a release, whose fence is
-// paid once per publication by a warp that moves no data, not once per piece by the warps that do
-// (there it took 1.5 us of a piece's 4 us).
-// W workers keep W pieces of each end in flight, so an end is bound by bytes in flight over the
-// ring round trip and not by one warp's copy latency.  The ring stays in L2; DRAM sees the
-// source once and the sink once.
+// W values is through: that minimum is the CTA's FRONTIER.  One more warp, the COMMITTER, keeps
+// taking the minimum (one value per lane, a warp shuffle reduction) and publishes it: "payload
+// first, then the counter".  Head needs a device-scope fence between the bulk writes and the
+// publication (without it the other end reads stale ring bytes: measured); it is taken by the
+// committer once per publication, or by each worker for its own piece where the ring's lap binds.
+// Tail needs none: the ring reads behind it have landed.  With several CTAs per end the other end
+// takes the minimum over the E frontiers it was told.  The ring stays in L2; DRAM sees the source
+// once and the sink once.
 //
 // Requires T % 16 == 0 and 16 B-aligned ring, source and sink addresses (bulk copies) and a
 // piece of at least kPipeMinPiece bytes; other shapes take the vector-copy kernels of hicr_channel.cu.
@@ -59,7 +62,7 @@ __device__ __forceinline__ void st_release_cta_shared_u64(unsigned long long *p,
     asm volatile("st.release.cta.shared::cta.u64 [%0], %1;" ::"r"(smem_u32(p)), "l"(v) : "memory");
 }
 
-// ---- thread-block cluster of two: the producer CTA (rank 0) and the consumer CTA (rank 1) of a ring
+// ---- thread-block cluster: the producer CTAs and the consumer CTAs of one ring
 __device__ __forceinline__ unsigned cluster_ctarank()
 {
     unsigned r;
