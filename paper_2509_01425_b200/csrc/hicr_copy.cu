@@ -223,7 +223,12 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // round trip overlaps the slot-table fetch and the shared-memory set-up
     uint4 alo = make_uint4(0, 0, 0, 0), ahi = alo;
     const uint64_t tile0 = (uint64_t)blockIdx.x * kThreads;
-    if (tile0 + tid < a.n) load_desc_raw(a.descs + tile0 + tid, alo, ahi);
+    // A table the host has validated and that holds no large descriptor needs no pass of its own over the
+    // descriptors: nothing to check, nothing to bin, and the messages are counted by the warp that copies
+    // them (phase B2) -- so the copies start with the kernel, and a table that is read in place from pinned
+    // host memory is fetched ticket by ticket behind them instead of once up front over PCIe.
+    const bool lazy = a.skip_barrier && use_hist;
+    if (!lazy && tile0 + tid < a.n) load_desc_raw(a.descs + tile0 + tid, alo, ahi);
     // ---- warp tickets of phase B2.  The first ticket of every warp is static (warp g owns
     // descriptors [g c0, (g+1) c0)); the others are atomics on a shared cursor that counts
     // from the end of the static tickets.
@@ -265,7 +270,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // ================================================================ phase A (a2, a3, a6)
     bool bad_seen = false;
     unsigned small_bytes = 0, small_cnt = 0;
-    for (uint64_t tile = tile0; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
+    for (uint64_t tile = lazy ? a.n : tile0; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
         const uint64_t i = tile + tid;
         uint64_t src = 0, dst = 0, size = 0;
         uint32_t ss = 0, ds = 0;
@@ -356,11 +361,21 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // ================================================================ grid barrier
     uint64_t src = 0, dst = 0;
     unsigned sz32 = 0;
+    // (a6, lazy tables) one message per descriptor of a ticket, counted by the warp that holds it: the lanes
+    // with the same slot elect one leader, which adds their number to the shared-memory histogram
+    auto count_ticket = [&](bool have, const uint4 &lo) {
+        const uint32_t ds_ = lo.x & kSlotIndexMask, ss_ = lo.y & kSlotIndexMask;
+        const unsigned ms = __match_any_sync(0xffffffffu, have ? ss_ : 0xffffffffu);
+        if (have && lane == __ffs(ms) - 1) atomicAdd(&hist[ss_], __popc(ms));
+        const unsigned md = __match_any_sync(0xffffffffu, have ? ds_ : 0xffffffffu);
+        if (have && lane == __ffs(md) - 1) atomicAdd(&hist[n_slots + ds_], __popc(md));
+    };
     if (fhave) {
         uint64_t size;
         uint32_t ds, ss;
         if (resolve(flo, fhi, cache, a.slots, n_slots, ds, ss, dst, src, size) == 0 && size <= kSmallMax) sz32 = (unsigned)size;
     }
+    if (lazy) count_ticket(fhave, flo);
     unsigned long long sync = 0;
     if (a.skip_barrier) {
         // host-validated table without large descriptors: nothing to agree on, nothing to wait for
@@ -397,21 +412,25 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         __syncthreads();
         sync = sh_sync;
     }
+    // the CTA's histogram into the cumulative counters: one atomic per touched slot
+    auto flush_hist = [&]() {
+        for (uint32_t s = tid; s < 2 * n_slots; s += kThreads) {
+            const unsigned v = hist[s];
+            if (!v) continue;
+            const uint32_t row = s < n_slots ? s : s - n_slots;
+            atomicAdd(s < n_slots ? &a.cnt[row].sent : &a.cnt[row].recv, (unsigned long long)v);
+            // a message on a global slot also counts at the slot's owner (published by the last CTA)
+            if (a.any_global && (slot_row(cache, a.slots, n_slots, row).meta & kRowGlobal))
+                atomicAdd(s < n_slots ? &a.gdelta[row].sent : &a.gdelta[row].recv, (unsigned long long)v);
+        }
+    };
     const bool ok = ((sync >> kSyncBadShift) & kSyncFieldMask) == 0;
     if (blockIdx.x == 0 && tid == 0) ctl->t_mid = globaltimer();
 
     if (ok) {
         // ============================================================ counters (a6)
         if (use_hist) {
-            for (uint32_t s = tid; s < 2 * n_slots; s += kThreads) {
-                const unsigned v = hist[s];
-                if (!v) continue;
-                const uint32_t row = s < n_slots ? s : s - n_slots;
-                atomicAdd(s < n_slots ? &a.cnt[row].sent : &a.cnt[row].recv, (unsigned long long)v);
-                // a message on a global slot also counts at the slot's owner (published by the last CTA)
-                if (a.any_global && (slot_row(cache, a.slots, n_slots, row).meta & kRowGlobal))
-                    atomicAdd(s < n_slots ? &a.gdelta[row].sent : &a.gdelta[row].recv, (unsigned long long)v);
-            }
+            if (!lazy) flush_hist();
         } else {
             // slot table too large for the shared-memory histogram: count straight into the
             // cumulative counters, now that the batch is known to be valid
@@ -558,6 +577,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
             }
             // rotate: k+1 becomes current (its descriptors have landed), k+2 starts loading
             sz32 = nhave ? resolve_small(nlo, nhi, cache, a.slots, n_slots, dst, src) : 0u;
+            if (lazy) count_ticket(nhave, nlo);
             first0 = first1;
             first1 = __shfl_sync(0xffffffffu, first2, 0);
             cnt1 = __shfl_sync(0xffffffffu, cnt2, 0);
@@ -569,6 +589,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
 
     // ================================================================ finish (feeds a7)
     __syncthreads();
+    if (lazy) {   // every warp has counted the tickets it copied
+        flush_hist();
+        __syncthreads();
+    }
     if (tid == 0) {
         sh_flag = atom_inc_acq_rel_u32(&ctl->done) == gridDim.x - 1;
         if (sh_flag) sh_seq = __ldcg(&ctl->seq) + 1;   // batches of a context run one after the other: one writer
