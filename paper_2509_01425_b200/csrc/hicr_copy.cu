@@ -240,6 +240,10 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     const unsigned static_end = nw * cnt_static;
     // ... and so are the descriptors of this warp's static first ticket: their round trip (cold: another
     // CTA's tile) hides behind phase A instead of sitting between it and the arrival at the barrier
+    // ... and so is the CTA's ticket for its warps' second tickets: an index range only, and an L2 round
+    // trip the arrival at the barrier would otherwise wait for (a release waits for the thread's own atomic)
+    unsigned cnt1 = a.hand_out != kHandOutStatic ? ticket_size(n, static_end) : 0u, base1 = 0;
+    if (tid == 0 && a.hand_out != kHandOutStatic) base1 = atomicAdd(&ctl->next_desc, cnt1 * kWarps);
     const unsigned first0_early = (blockIdx.x * kWarps + warp) * cnt_static;
     uint4 flo = make_uint4(0, 0, 0, 0), fhi = flo;
     const bool fhave = (unsigned)lane < cnt_static && first0_early + lane < n;
@@ -268,7 +272,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     __syncthreads();
 
     // ================================================================ phase A (a2, a3, a6)
-    bool bad_seen = false;
+    bool bad_seen = false, wrote_chunks = false;
     unsigned small_bytes = 0, small_cnt = 0;
     for (uint64_t tile = lazy ? a.n : tile0; tile < a.n; tile += (uint64_t)gridDim.x * kThreads) {
         const uint64_t i = tile + tid;
@@ -303,6 +307,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         const bool is_large = valid && size > kSmallMax;
         const unsigned large_mask = __ballot_sync(0xffffffffu, is_large);
         if (large_mask) {
+            wrote_chunks = true;
             const unsigned nch = is_large ? chunk_count(dst, size) : 0u;
             unsigned incl = nch;   // inclusive warp scan of the chunk counts
 #pragma unroll
@@ -355,8 +360,6 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
     // (ONE atomic per CTA for its eight warps' second tickets: 2368 same-address atomics at once
     // take microseconds to drain, and the CTA's arrival at the barrier waits for its own)
     unsigned first0 = (blockIdx.x * kWarps + warp) * cnt_static, first1 = 0;
-    unsigned cnt1 = a.hand_out != kHandOutStatic ? ticket_size(n, static_end) : 0u, base1 = 0;
-    if (tid == 0 && a.hand_out != kHandOutStatic) base1 = atomicAdd(&ctl->next_desc, cnt1 * kWarps);
 
     // ================================================================ grid barrier
     uint64_t src = 0, dst = 0;
@@ -386,10 +389,15 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) engine_kernel(const Engi
         // without arriving (a 256-descriptor batch is a barrier of one arrival, not 296)
         const unsigned arrivals = min((unsigned)gridDim.x, (n + kThreads - 1) / kThreads);
         const int cta_bad = __syncthreads_or(bad_seen);
+        const int cta_chunks = __syncthreads_or(wrote_chunks);
         if (tid == 0 && blockIdx.x < arrivals) {
             const unsigned long long vote = sh_small[1] != 0 && sh_small[0] <= (unsigned long long)(kTeamMax / 16) * sh_small[1];
-            atom_add_release_u64(&ctl->sync, 1ull | ((unsigned long long)(cta_bad != 0) << kSyncBadShift) |
-                                                 (vote << kSyncVoteShift));
+            const unsigned long long word = 1ull | ((unsigned long long)(cta_bad != 0) << kSyncBadShift) | (vote << kSyncVoteShift);
+            // the arrival releases what the other CTAs will read after the barrier: this CTA's chunk-queue
+            // items.  A CTA that wrote none has nothing to release (its verdict and vote travel in the word
+            // itself), and a relaxed add spares it the fence of a release
+            if (cta_chunks) atom_add_release_u64(&ctl->sync, word);
+            else asm volatile("red.relaxed.gpu.global.add.u64 [%0], %1;" ::"l"(&ctl->sync), "l"(word) : "memory");
         }
         // While the barrier fills, the sources of the first descriptors this warp will copy start
         // moving into L2, one 128-byte line per lane: the DRAM would otherwise idle until the
