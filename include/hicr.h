@@ -187,6 +187,65 @@ int hicr_graph_destroy(hicr_graph_t *g);
  * which descriptor index in it was the first bad one.  Host pointers out (may be NULL). */
 int hicr_fence_error(hicr_ctx_t *ctx, uint64_t *batch_index, uint64_t *first_bad);
 
+/* ---- memcpy for callers that cannot allocate ---------------------------------
+ *
+ * hicr_init and hicr_memcpy_batch allocate: the context's tables at start, and the engine's chunk
+ * queue again (cudaFree + cudaMalloc, which stall the whole device) whenever a batch is larger
+ * than any before it.  That rules the context path out for a process whose HBM was given to its
+ * own pool at start-up (a serving engine, a framework's caching allocator: a library's cudaMalloc
+ * then fails), and for a step loop with a latency budget that shares the GPU with other streams
+ * (they all wait while cudaMalloc / cudaFree run).  This one call is for them.  It needs no
+ * context and allocates nothing, on the device or on the host: its work memory -- control words,
+ * a per-slot count histogram and the chunk queue -- is one array of about 1 MiB built into the
+ * library's device code, which every GPU that runs this library holds until the process exits.
+ *
+ * One batch, start to end, enqueued on `cuda_stream` (a cudaStream_t of `device`; NULL = the
+ * legacy default stream): validate all n descriptors, then -- only if all are valid -- carry out
+ * dst[dst_off + i] = src[src_off + i] for each and count one message per descriptor.  It is
+ * asynchronous and there is no fence: everything it writes is complete and visible to whatever
+ * the caller orders after it on the stream.
+ *
+ *   d_slots     device pointer, n_slots rows {base, size}; a descriptor's dst_slot / src_slot is an
+ *               index into it.  base: device pointer, any alignment.
+ *   d_descs     device pointer, n descriptors; unchanged until the call's work is done.
+ *   d_counters  device pointer, 2 * n_slots words, in/out: [2 s] += messages whose source was
+ *               slot s, [2 s + 1] += messages whose destination was slot s.  The caller zeroes it
+ *               once; calls accumulate, as hicr_slot_counters does.
+ *   d_result    device pointer, 2 words, out: [0] = HICR_OK, or the status of the lowest bad
+ *               descriptor (HICR_ERR_INVALID_SLOT: index >= n_slots; HICR_ERR_OUT_OF_BOUNDS;
+ *               destination checked before source), [1] = that descriptor's index.  On an error
+ *               nothing was copied and nothing counted, as for hicr_memcpy_batch.
+ *
+ * Limits, because the work memory cannot grow: n <= HICR_NOALLOC_MAX_DESCS and
+ * n_slots <= HICR_NOALLOC_MAX_SLOTS, else HICR_ERR_NO_CAPACITY is returned and nothing is
+ * enqueued.  Descriptors above 8 KiB are cut into 128 KiB chunks (size / 128 KiB, rounded up); a
+ * batch may hold HICR_NOALLOC_MAX_CHUNKS of them (4 GiB of large transfers).  Only the device sees the
+ * sizes, so one chunk too many comes back as d_result[0] = HICR_ERR_NO_CAPACITY with the index
+ * of a descriptor that did not fit, and again nothing is copied.
+ *
+ * Sharing: every call in the process that targets `device` uses the same array, and the array
+ * keeps the previous call's contents; each call first clears, in stream order, the part that
+ * must start at zero.  Calls on one stream, or otherwise ordered one after the other, are safe.
+ * Calls that can run on the GPU at the same time (two streams, no event between them) race on
+ * the array: undefined results.
+ *
+ * The first call for a device looks up where the array sits on that device (once; later calls
+ * reuse the address).  Make that first call before any stream capture is in progress.
+ *
+ * Same caller contract as hicr_memcpy_batch: destination ranges of one batch pairwise disjoint
+ * and disjoint from every source range.  Global slots, host-resident tables and profiling belong
+ * to the context path only.  Returns HICR_OK once enqueued, HICR_ERR_INVALID_ARG (NULL where
+ * needed, device out of range), HICR_ERR_NO_CAPACITY, HICR_ERR_CUDA. */
+#define HICR_NOALLOC_MAX_DESCS  65536u
+#define HICR_NOALLOC_MAX_SLOTS  1024u
+#define HICR_NOALLOC_MAX_CHUNKS 32768u
+typedef struct hicr_raw_slot {
+    void *base;       /* device pointer */
+    uint64_t size;    /* bytes */
+} hicr_raw_slot_t;
+int hicr_memcpy_batch_noalloc(int device, void *cuda_stream, const hicr_raw_slot_t *d_slots, uint32_t n_slots,
+                              const hicr_desc_t *d_descs, uint64_t n, uint64_t *d_counters, int64_t *d_result);
+
 /* ---- Global Memory Slots (S3.1.4) -------------
  *
  * "The communication manager also is in charge of creating and exchanging Global Memory Slots,

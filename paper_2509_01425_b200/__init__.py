@@ -22,12 +22,17 @@ from .binding import (  # noqa: F401
     HICR_GLOBAL_HANDLE_BYTES,
     GLOBAL_COUNT_DTYPE,
     HICR_MAX_SLOTS,
+    HICR_NOALLOC_MAX_CHUNKS,
+    HICR_NOALLOC_MAX_DESCS,
+    HICR_NOALLOC_MAX_SLOTS,
     HICR_OK,
     LIB_PATH,
     Channel,
     Context,
     HicrError,
     Mpsc,
+    RAW_SLOT_DTYPE,
     lib,
+    memcpy_batch_noalloc,
 )
 from . import collective  # noqa: F401,E402

@@ -46,6 +46,7 @@ EXPORTS = (
     "hicr_init", "hicr_finalize", "hicr_strerror", "hicr_last_cuda_error",
     "hicr_slot_register", "hicr_slot_unregister", "hicr_slot_counters",
     "hicr_memcpy_batch", "hicr_fence", "hicr_fence_error", "hicr_fence_async", "hicr_fence_expected",
+    "hicr_memcpy_batch_noalloc",
     "hicr_channel_create", "hicr_channel_destroy", "hicr_channel_counters",
     "hicr_channel_push", "hicr_channel_pop", "hicr_channel_stream",
     "hicr_mpsc_create", "hicr_mpsc_destroy", "hicr_mpsc_counters", "hicr_mpsc_stream",
@@ -74,6 +75,7 @@ def _load() -> ctypes.CDLL:
         "hicr_slot_unregister": (i32, [vp, u32]),
         "hicr_slot_counters": (i32, [vp, u32, P(u64), P(u64)]),
         "hicr_memcpy_batch": (i32, [vp, vp, u64, i32, P(u64)]),
+        "hicr_memcpy_batch_noalloc": (i32, [i32, vp, vp, u32, vp, u64, vp, vp]),
         "hicr_fence": (i32, [vp]),
         "hicr_fence_error": (i32, [vp, P(u64), P(u64)]),
         "hicr_fence_async": (i32, [vp]),
@@ -128,6 +130,25 @@ class HicrError(RuntimeError):
         if detail:
             msg += " [" + detail + "]"
         super().__init__(msg)
+
+
+# hicr_raw_slot_t: one row of the slot array hicr_memcpy_batch_noalloc takes
+RAW_SLOT_DTYPE = np.dtype([("base", "<u8"), ("size", "<u8")])
+HICR_NOALLOC_MAX_DESCS = 65536
+HICR_NOALLOC_MAX_SLOTS = 1024
+HICR_NOALLOC_MAX_CHUNKS = 32768
+
+
+def memcpy_batch_noalloc(device: int, stream: int, d_slots: int, n_slots: int, d_descs: int, n: int,
+                         d_counters: int, d_result: int) -> None:
+    """hicr_memcpy_batch_noalloc: the batch for callers that may not allocate (a process whose
+    HBM belongs to its own pool, a loop that cannot take cudaMalloc's device-wide stall).  All
+    pointers are device addresses as ints (``tensor.data_ptr()``); ``stream`` a cudaStream_t as
+    int.  Enqueues and returns; status and first bad index arrive in ``d_result``.  Raises
+    HicrError for what the host can refuse (limits, NULL, CUDA errors)."""
+    rc = lib.hicr_memcpy_batch_noalloc(device, stream, d_slots, n_slots, d_descs, n, d_counters, d_result)
+    if rc != HICR_OK:
+        raise HicrError(rc, "hicr_memcpy_batch_noalloc")
 
 
 def _slot_ids(ids) -> np.ndarray:
