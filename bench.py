@@ -855,7 +855,19 @@ def run_channel(args):
     return 0
 
 
+def spawn_command(n_gpus, argv, port=None):
+    """The launch line of the contract: one rank per GPU of this node, rendezvous on 127.0.0.1."""
+    if port is None:
+        import socket
+        with socket.socket() as s:
+            s.bind(("127.0.0.1", 0))
+            port = s.getsockname()[1]
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n_gpus),
+            "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
+
+
 def main(argv=None):
+    argv = list(sys.argv[1:] if argv is None else argv)
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=2000)
@@ -877,6 +889,14 @@ def main(argv=None):
         return run_channel(args)
     if args.impl == "reference":
         return run_reference(args)
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # `python bench.py --gpus N` without a launcher: start the N ranks ourselves (the same line the
+        # driver uses); rank 0 of them prints the JSON line
+        import subprocess
+        import torch
+        if torch.cuda.device_count() < args.gpus:
+            raise SystemExit("bench.py: --gpus %d but this node has %d CUDA device(s)" % (args.gpus, torch.cuda.device_count()))
+        return subprocess.call(spawn_command(args.gpus, argv))
     return run_cuda(args)
 
 

@@ -68,3 +68,25 @@ def test_two_ranks_shard_and_aggregate(tmp_path):
 def test_rank_max_single_process():
     import bench
     assert bench.rank_max(3.5) == 3.5
+
+
+def test_gpus_flag_without_a_launcher_starts_the_ranks(monkeypatch):
+    """`python bench.py --gpus N` on its own must not run one rank and call it N: without
+    WORLD_SIZE in the environment it re-launches itself as N ranks with the contract's line."""
+    import subprocess
+
+    import bench
+    cmd = bench.spawn_command(4, ["--gpus", "4", "--steps", "5"], port=29511)
+    assert cmd[1:4] == ["-m", "torch.distributed.run", "--nnodes=1"]
+    assert cmd[cmd.index("--nproc-per-node") + 1] == "4"
+    assert cmd[cmd.index("--master-addr") + 1] == "127.0.0.1" and cmd[cmd.index("--master-port") + 1] == "29511"
+    assert cmd[-5:] == [os.path.join(ROOT, "bench.py"), "--gpus", "4", "--steps", "5"]
+    monkeypatch.delenv("WORLD_SIZE", raising=False)
+    seen = []
+    monkeypatch.setattr(subprocess, "call", lambda c: seen.append(c) or 0)
+    monkeypatch.setattr(torch.cuda, "device_count", lambda: 2)
+    assert bench.main(["--gpus", "2", "--steps", "3", "--warmup", "3"]) == 0
+    assert len(seen) == 1 and seen[0][-6:] == ["--gpus", "2", "--steps", "3", "--warmup", "3"]
+    with pytest.raises(SystemExit) as e:
+        bench.main(["--gpus", "8"])                      # more ranks than devices: refused, not shrunk
+    assert "8" in str(e.value) and not seen[1:]
