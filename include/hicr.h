@@ -171,8 +171,10 @@ int hicr_fence_expected(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t sent, uint64
  * Every replay validates, bins, copies and counts on the device exactly like the calls it
  * records; completion, counters and deferred errors come with the next blocking hicr_fence,
  * whose batch_index counts the batches since the last blocking fence as usual.  The tables must
- * stay alive and the slot table unchanged from hicr_graph_begin to the last launch
- * (HICR_ERR_INVALID_ARG from hicr_graph_launch otherwise).  While recording, every other call
+ * stay alive and the slot table unchanged from hicr_graph_begin to the last launch, and no
+ * hicr_memcpy_batch after the recording may be larger than every batch before it and than
+ * max_descs_per_batch (that re-allocates the work queue the recorded launches name):
+ * HICR_ERR_INVALID_ARG from hicr_graph_launch otherwise.  While recording, every other call
  * that would enqueue work on the stream returns HICR_ERR_BUSY.  A chain holds at most 64 batches
  * (HICR_ERR_NO_CAPACITY); max_descs_per_batch sizes the work queues up front.  The context must
  * have been created on a stream of its own (HICR_ERR_INVALID_ARG on the legacy default stream,

@@ -413,6 +413,7 @@ int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes,
     if (!ctx || !out) return HICR_ERR_INVALID_ARG;
     *out = nullptr;
     if (token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;   // capacity >= 1
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     const int64_t ri = slot_find(ctx, ring);
     if (ri < 0) return HICR_ERR_INVALID_SLOT;
     if (!tokens_fit(capacity, token_bytes, 0, row_size(ctx->rows[ri]))) return HICR_ERR_OUT_OF_BOUNDS;
@@ -438,6 +439,7 @@ int hicr_channel_create(hicr_ctx_t *ctx, hicr_slot_t ring, uint64_t token_bytes,
 int hicr_channel_destroy(hicr_channel_t *ch)
 {
     if (!ch) return HICR_ERR_INVALID_ARG;
+    if (ch->ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     (void)cudaStreamSynchronize(ch->ctx->stream);
     cudaFree(ch->d_state);
     cudaFree(ch->d_tab);
@@ -461,6 +463,7 @@ static int channel_call(hicr_channel_t *ch, bool push, hicr_slot_t lin_slot, uin
 {
     if (!ch || !n_out) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = ch->ctx;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     *n_out = 0;
     const int64_t li = slot_find(ctx, lin_slot);
     if (li < 0) return HICR_ERR_INVALID_SLOT;
@@ -560,6 +563,7 @@ int hicr_channel_stream(hicr_channel_t *ch, hicr_slot_t src, uint64_t src_off, h
 {
     if (!ch || (!batch_tokens && n_batches)) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = ch->ctx;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     const int64_t si = slot_find(ctx, src), di = slot_find(ctx, dst);
     if (si < 0 || di < 0) return HICR_ERR_INVALID_SLOT;
     if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;
@@ -627,6 +631,7 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
 {
     if (!ctx || !out || !rings) return HICR_ERR_INVALID_ARG;
     *out = nullptr;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     if (producers == 0 || token_bytes == 0 || capacity == 0) return HICR_ERR_INVALID_ARG;
     std::vector<uint32_t> idx(producers);
     for (uint32_t p = 0; p < producers; p++) {
@@ -663,6 +668,7 @@ int hicr_mpsc_create(hicr_ctx_t *ctx, uint32_t producers, const hicr_slot_t *rin
 int hicr_mpsc_destroy(hicr_mpsc_t *m)
 {
     if (!m) return HICR_ERR_INVALID_ARG;
+    if (m->ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     (void)cudaStreamSynchronize(m->ctx->stream);
     cudaFree(m->d_state);
     cudaFree(m->d_ptrs);
@@ -685,6 +691,7 @@ int hicr_mpsc_stream(hicr_mpsc_t *m, const hicr_slot_t *src_slots, const uint64_
 {
     if (!m || !src_slots || !dst_slots || max_batch == 0) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = m->ctx;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     const uint32_t P = m->P;
     const uint64_t N = tokens_per_producer;
     if (N > (1ull << 48) / m->T) return HICR_ERR_OUT_OF_BOUNDS;
@@ -765,6 +772,7 @@ int hicr_mpsc_locking_stream(hicr_channel_t *ch, uint32_t producers, const hicr_
 {
     if (!ch || !src_slots || producers == 0 || max_batch == 0) return HICR_ERR_INVALID_ARG;
     hicr_ctx *ctx = ch->ctx;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     const uint32_t P = producers;
     const uint64_t N = tokens_per_producer;
     if (ch->head != ch->tail) return HICR_ERR_INVALID_ARG;   // requires an empty ring at entry

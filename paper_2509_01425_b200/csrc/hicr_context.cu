@@ -198,6 +198,9 @@ int slot_install(hicr_ctx *ctx, uint64_t base, uint64_t size, uint64_t flags, hi
     HICR_CUDA(ctx, cudaMemcpyAsync(ctx->d_slots + i, &row, sizeof(row), cudaMemcpyHostToDevice, ctx->stream));
     if (reuse) {
         HICR_CUDA(ctx, cudaMemsetAsync(ctx->d_cnt + i, 0, sizeof(SlotCnt), ctx->stream));
+        // owner-side totals of an earlier registration that was volunteered under this index: a new
+        // slot starts at zero there too (an index never handed out before still is zero)
+        if (ctx->d_gcnt) HICR_CUDA(ctx, cudaMemsetAsync(ctx->d_gcnt + i, 0, sizeof(SlotCnt), ctx->stream));
         ctx->free_idx.pop_back();
         ctx->rows[i] = row;
         ctx->gen[i] = g;

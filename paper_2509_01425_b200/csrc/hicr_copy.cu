@@ -677,6 +677,7 @@ static int ensure_queues(hicr_ctx *ctx, uint64_t n)
         ctx->chunk_cap = 0;
         HICR_CUDA(ctx, cudaMalloc(&ctx->d_chunk, cap * sizeof(WorkItem)));
         ctx->chunk_cap = cap;
+        ctx->queue_version++;   // recorded chains name the old queue: hicr_graph_launch refuses them
     }
     return HICR_OK;
 }
@@ -901,7 +902,7 @@ struct hicr_graph {
     cudaGraph_t graph = nullptr;
     cudaGraphExec_t exec = nullptr;
     uint32_t n_batches = 0, n_push = 0;
-    uint64_t table_version = 0;
+    uint64_t table_version = 0, queue_version = 0;
 };
 
 extern "C" int hicr_graph_begin(hicr_ctx_t *ctx, uint64_t max_descs_per_batch)
@@ -929,6 +930,7 @@ extern "C" int hicr_graph_end(hicr_ctx_t *ctx, hicr_graph_t **out)
     g->n_batches = ctx->captured_batches;
     g->n_push = std::min<uint32_t>((uint32_t)ctx->rows.size(), kPushSlots);
     g->table_version = ctx->table_version;
+    g->queue_version = ctx->queue_version;
     cudaError_t e = cudaStreamEndCapture(ctx->stream, &g->graph);
     if (e == cudaSuccess && g->graph) e = cudaGraphInstantiate(&g->exec, g->graph, 0);
     if (e != cudaSuccess || !g->graph) {
@@ -946,6 +948,7 @@ extern "C" int hicr_graph_launch(hicr_graph_t *g)
     hicr_ctx *ctx = g->ctx;
     if (ctx->capturing) return HICR_ERR_BUSY;
     if (g->table_version != ctx->table_version) return HICR_ERR_INVALID_ARG;   // the recorded launches name another slot table
+    if (g->queue_version != ctx->queue_version) return HICR_ERR_INVALID_ARG;   // ... or a chunk queue that has been freed since
     if (g->n_batches == 0) return HICR_OK;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     if (ctx->batches_in_epoch + g->n_batches > (uint32_t)kRecRing) {

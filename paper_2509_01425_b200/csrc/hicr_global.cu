@@ -244,6 +244,7 @@ int hicr_global_volunteer(hicr_ctx_t *ctx, uint64_t tag, uint64_t key, hicr_slot
 int hicr_global_exchange(hicr_ctx_t *ctx, uint64_t tag, const hicr_global_handle_t *handles, uint64_t n, hicr_slot_t *out_slots)
 {
     if (!ctx || ((!handles || !out_slots) && n)) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     if (n == 0) return HICR_OK;
     GlobalTable *g = ctx->globals;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
@@ -332,11 +333,12 @@ int hicr_global_lookup(hicr_ctx_t *ctx, uint64_t tag, uint64_t key, hicr_slot_t 
 int hicr_global_fence_begin(hicr_ctx_t *ctx, hicr_global_count_t *out, uint64_t cap, uint64_t *n)
 {
     if (!ctx || !n || (!out && cap)) return HICR_ERR_INVALID_ARG;
-    const int frc = hicr_fence(ctx);
-    if (frc == HICR_ERR_CUDA) return frc;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     GlobalTable *g = ctx->globals;
     *n = g->by_index.size();
-    if (*n > cap) return HICR_ERR_NO_CAPACITY;
+    if (*n > cap) return HICR_ERR_NO_CAPACITY;   // before the fence: a retry with more room still gets the epoch's deferred error
+    const int frc = hicr_fence(ctx);
+    if (frc == HICR_ERR_CUDA) return frc;
     uint64_t k = 0;
     for (auto &kv : g->by_index) {
         out[k].tag = kv.second.tag;
@@ -351,6 +353,7 @@ int hicr_global_fence_begin(hicr_ctx_t *ctx, hicr_global_count_t *out, uint64_t 
 int hicr_global_fence_end(hicr_ctx_t *ctx, const hicr_global_count_t *all, uint64_t n_all, uint32_t timeout_ms)
 {
     if (!ctx || (!all && n_all)) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     GlobalTable *g = ctx->globals;
     HICR_CUDA(ctx, cudaSetDevice(ctx->device));
     // the expected totals of every global slot this context owns: the sums of its lines
@@ -382,6 +385,7 @@ int hicr_global_fence_end(hicr_ctx_t *ctx, const hicr_global_count_t *all, uint6
 int hicr_global_counters(hicr_ctx_t *ctx, hicr_slot_t slot, uint64_t *sent, uint64_t *recv)
 {
     if (!ctx || !sent || !recv) return HICR_ERR_INVALID_ARG;
+    if (ctx->capturing) return HICR_ERR_BUSY;   // a chain is being recorded on the stream (hicr_graph_begin)
     int64_t i = slot_find(ctx, slot);
     if (i < 0) return HICR_ERR_INVALID_SLOT;
     if (ctx->rows[i].meta & kRowGlobal) {

@@ -630,6 +630,7 @@ struct hicr_ctx {
     bool capturing = false;
     uint32_t captured_batches = 0;
     uint64_t table_version = 0;              // bumped by every change of the slot table
+    uint64_t queue_version = 0;              // bumped whenever the chunk queue is re-allocated
 
     void *launch_cache = nullptr;            // hicr_copy.cu: instantiated one-kernel graphs of recent engine launches
 

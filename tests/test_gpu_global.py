@@ -20,6 +20,7 @@ import oracle
 import workloads as W
 from global_common import NAMES, descs_for, oracle_run
 from oracle.world import World
+from parity import to_device_table
 
 pytestmark = pytest.mark.gpu
 
@@ -305,3 +306,73 @@ def test_two_processes_over_cuda_ipc():
     for r, (p, out) in enumerate(zip(procs, outs)):
         assert p.returncode == 0, "rank %d:\n%s" % (r, out[-3000:])
         assert "global two-process parity ok" in out
+
+
+def test_recycled_index_starts_with_zero_owner_totals(hicr):
+    """The owner-side totals belong to a registration, not to a table index: a slot registered at
+    an index whose earlier slot had been volunteered starts at (0, 0), as the oracle's does
+    (oracle_slot_register zeroes them), and the global fence waits for the NEW slot's transfers."""
+    world = World(2)
+    ctxs = _instances(hicr, 2)
+    try:
+        imgs = [np.zeros(4096, dtype=np.uint8), (np.arange(4096) % 251).astype(np.uint8)]
+        o_imgs = [i.copy() for i in imgs]
+        bufs = [torch.from_numpy(i).cuda() for i in imgs]
+        sa, sb = ctxs[0].slot_register(bufs[0]), ctxs[1].slot_register(bufs[1])
+        oa, ob = world.inst[0].slot_register(o_imgs[0]), world.inst[1].slot_register(o_imgs[1])
+        out = hicr.collective.exchange_in_process(ctxs, 1, [[(0, sa)], []])
+        rc, oout = world.exchange(1, [[(0, oa)], []])
+        assert rc == oracle.OK
+        put5 = lambda g, s: W.make_descs([g] * 5, [s] * 5, [0, 100, 200, 300, 400], [7, 9, 11, 13, 15], [64] * 5)
+        ctxs[1].memcpy_batch(put5(out[1][0], sb))
+        hicr.collective.fence_in_process(ctxs)
+        assert world.inst[1].memcpy_batch(put5(oout[1][0], ob))[0] == oracle.OK
+        world.fence_all()
+        assert ctxs[0].global_counters(sa) == world.inst[0].slot_global_counters(oa) == (0, 5)
+        # drop the global slot everywhere, then the local slot behind it; the index comes back
+        for c, o in zip(ctxs, out):
+            c.slot_unregister(o[0])
+        ctxs[0].slot_unregister(sa)
+        assert world.inst[0].slot_unregister(oa) == oracle.OK
+        o_new = np.zeros(4096, dtype=np.uint8)
+        new = torch.from_numpy(o_new.copy()).cuda()
+        sa2, oa2 = ctxs[0].slot_register(new), world.inst[0].slot_register(o_new)
+        assert sa2 != sa and (sa2 & 0xfff) == (sa & 0xfff)
+        assert ctxs[0].global_counters(sa2) == world.inst[0].slot_global_counters(oa2) == (0, 0)
+        out2 = hicr.collective.exchange_in_process(ctxs, 2, [[(0, sa2)], []])
+        rc, oout2 = world.exchange(2, [[(0, oa2)], []])
+        assert rc == oracle.OK
+        two = lambda g, s: W.make_descs([g] * 2, [s] * 2, [5, 1000], [0, 2000], [333, 777])
+        ctxs[1].memcpy_batch(two(out2[1][0], sb))
+        hicr.collective.fence_in_process(ctxs)
+        assert world.inst[1].memcpy_batch(two(oout2[1][0], ob))[0] == oracle.OK
+        world.fence_all()
+        assert ctxs[0].global_counters(sa2) == world.inst[0].slot_global_counters(oa2) == (0, 2)
+        assert new.cpu().numpy().tobytes() == o_new.tobytes()
+    finally:
+        _close(ctxs)
+
+
+def test_global_fence_keeps_the_error_with_more_than_64_global_slots(hicr):
+    """hicr_global_fence_begin reports how much room it needs BEFORE it fences, so the retry with
+    a larger array still returns the epoch's deferred error (66 global slots, one bad descriptor)."""
+    ctxs = _instances(hicr, 2)
+    try:
+        bufs = [[torch.zeros(256, dtype=torch.uint8, device="cuda") for _ in range(33)] for _ in ctxs]
+        ids = [[c.slot_register(b) for b in bb] for c, bb in zip(ctxs, bufs)]
+        out = hicr.collective.exchange_in_process(ctxs, 3, [[(k, s) for k, s in enumerate(ids[0])],
+                                                            [(100 + k, s) for k, s in enumerate(ids[1])]])
+        assert len(out[0]) == 66
+        bad = W.make_descs([out[0][100], out[0][101]], [ids[0][0], ids[0][1]], [0, 200], [0, 0], [16, 64])   # second: out of bounds
+        t = to_device_table(bad)
+        ctxs[0].memcpy_batch(t, n=2)
+        with pytest.raises(hicr.HicrError) as e:
+            hicr.collective.fence_in_process(ctxs)
+        assert (e.value.status, e.value.first_bad) == (hicr.HICR_ERR_OUT_OF_BOUNDS, 1)
+        assert ctxs[1].global_counters(ids[1][0]) == (0, 0)
+        good = W.make_descs([out[0][100]], [ids[0][0]], [0], [0], [16])
+        ctxs[0].memcpy_batch(good)
+        hicr.collective.fence_in_process(ctxs)
+        assert ctxs[1].global_counters(ids[1][0]) == (0, 1)
+    finally:
+        _close(ctxs)

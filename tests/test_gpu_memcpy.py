@@ -750,3 +750,80 @@ def test_randomized_mixes(hicr):
             got = run_gpu(w, device_tables=dev, split=int(rng.integers(1, 4)))
             assert_same(w, ref, got, "kind %d seed %d device_tables %s" % (kind, seed, dev))
         done += 1
+
+
+def test_chain_refused_after_the_chunk_queue_moved(hicr):
+    """A recorded chain names the chunk queue it was recorded with.  An ordinary batch larger than
+    anything before re-allocates that queue; the chain must then be refused, not replayed into
+    freed memory."""
+    MiB = W.MiB
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream), hicr.Context(0, stream.cuda_stream) as ctx:
+        a = torch.zeros(8 * MiB, dtype=torch.uint8, device="cuda")
+        b = torch.from_numpy(W.random_bytes(W.rng_for(9, 1), 8 * MiB)).cuda()
+        sa, sb = ctx.slot_register(a), ctx.slot_register(b)
+        large = W.make_descs([sa] * 4, [sb] * 4, [k * MiB + 3 for k in range(4)], [k * MiB + 5 for k in range(4)], [MiB - 64] * 4)
+        t = to_device_table(large)
+        stream.synchronize()
+        ctx.graph_begin(16)
+        ctx.memcpy_batch(t, n=4)
+        g = ctx.graph_end()
+        g.launch()
+        ctx.fence()
+        for k in range(4):
+            assert torch.equal(a[k * MiB + 3: (k + 1) * MiB - 61], b[k * MiB + 5: (k + 1) * MiB - 59])
+        # 20,000 descriptors: far more than the 16 the recording sized the queue for
+        many = W.make_descs([sa] * 20000, [sb] * 20000, np.arange(20000) * 64 + 4 * MiB, np.arange(20000) * 64, [48] * 20000)
+        t2 = to_device_table(many)
+        ctx.memcpy_batch(t2, n=20000)
+        ctx.fence()
+        with pytest.raises(hicr.HicrError) as e:
+            g.launch()
+        assert e.value.status == hicr.HICR_ERR_INVALID_ARG
+        ctx.fence()
+        g.close()
+        # a chain recorded now replays
+        ctx.graph_begin(16)
+        ctx.memcpy_batch(t, n=4)
+        g2 = ctx.graph_end()
+        a.zero_()
+        g2.launch()
+        ctx.fence()
+        assert torch.equal(a[3: MiB - 61], b[5: MiB - 59])
+        g2.close()
+
+
+def test_recording_refuses_channel_and_global_calls(hicr):
+    """While a chain is being recorded every other call that would put work on the stream
+    returns HICR_ERR_BUSY (hicr.h): channels, MPSC sets and the global-slot calls too."""
+    stream = torch.cuda.Stream()
+    with torch.cuda.stream(stream), hicr.Context(0, stream.cuda_stream) as ctx:
+        ring, src, dst = (torch.zeros(4096, dtype=torch.uint8, device="cuda") for _ in range(3))
+        r, s, d = (ctx.slot_register(x) for x in (ring, src, dst))
+        ch = ctx.channel_create(r, 64, 16)
+        r2 = ctx.slot_register(torch.zeros(4096, dtype=torch.uint8, device="cuda"))
+        m = ctx.mpsc_create([r2], 64, 16)
+        handle = ctx.global_volunteer(1, 0, s)
+        one = to_device_table(W.make_descs([d], [s], [1024], [0], [16]))
+        stream.synchronize()
+        ctx.graph_begin(16)
+        ctx.memcpy_batch(one, n=1)
+        refused = [
+            lambda: ch.push(s, 0, 4), lambda: ch.pop(d, 0, 4), lambda: ch.stream(s, 0, d, 0, [4, 4]),
+            lambda: ch.locking_stream([s], d, 0, 8, 4), lambda: m.stream([s], [d], 8, 4),
+            lambda: ctx.channel_create(r2, 64, 16), lambda: ctx.mpsc_create([r2], 64, 16),
+            lambda: ctx.global_fence_begin(), lambda: ctx.global_fence_end(np.zeros(1, dtype=hicr.GLOBAL_COUNT_DTYPE)),
+            lambda: ctx.global_counters(s), lambda: ctx.global_exchange(1, [handle]),
+        ]
+        for k, call in enumerate(refused):
+            with pytest.raises(hicr.HicrError) as e:
+                call()
+            assert e.value.status == hicr.HICR_ERR_BUSY, k
+        g = ctx.graph_end()
+        g.close()
+        # and the same calls work once the recording is over
+        src.copy_(torch.arange(4096, dtype=torch.int32, device="cuda").to(torch.uint8))
+        assert ch.push(s, 0, 4) == 4 and ch.pop(d, 0, 4) == 4
+        assert torch.equal(dst[:256], src[:256])
+        m.close()
+        ch.close()
