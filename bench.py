@@ -361,6 +361,70 @@ def cross_gpu_leg(hicr, ctx, rank, world, group, stream, steps=20, pages=16384, 
             "window_equals_peer_source": ok, "peer": peer}
 
 
+def other_configs_brief(hicr, torch, device, budget_s=20.0):
+    """BASELINE.json's metric names more than config 2 ("descriptors/s + fence"): the full-size configs 1 and 4,
+    each on a context and stream of its own, timed with CUDA events like `value`.  They ride in the default
+    line as `other_configs` so that whoever runs bench.py records them too; the 16 GiB configs (3a, 3b) and the
+    channel runs (5a, 5b) take too long to set up for that and keep their own --config runs."""
+    out = {}
+    t_all = time.perf_counter()
+    for name, what in (("tiny", "device"), ("chain", "device"), ("chain_graph", "graph")):
+        if time.perf_counter() - t_all > budget_s:
+            out[name] = {"skipped": "time budget of the side measurements used up"}
+            continue
+        try:
+            w = make_workload(name, 0)
+            stream = torch.cuda.Stream()
+            with torch.cuda.stream(stream):
+                ctx = hicr.Context(device, stream.cuda_stream)
+                try:
+                    bufs = [torch.from_numpy(w.slot_image(s)).cuda() for s in range(len(w.slot_sizes))]
+                    for b in bufs:
+                        ctx.slot_register(b)
+                    tabs = [torch.from_numpy(np.ascontiguousarray(e).view(np.uint8).copy()).cuda() for e in w.epochs]
+                    ptrs, n_per, n_sets = [t.data_ptr() for t in tabs], [len(e) for e in w.epochs], len(w.epochs)
+                    stream.synchronize()
+                    graph = None
+                    if what == "graph":
+                        ctx.graph_begin(max(n_per))
+                        for i in range(n_sets):
+                            ctx.memcpy_batch(ptrs[i], n_per[i])
+                            ctx.fence_async()
+                        graph = ctx.graph_end()
+
+                    def run(k):
+                        if graph is None:
+                            for i in range(k):
+                                ctx.memcpy_batch(ptrs[i % n_sets], n_per[i % n_sets])
+                                ctx.fence()
+                        else:
+                            for _ in range(k // n_sets):
+                                graph.launch()
+                                ctx.fence()
+
+                    K = 10 * n_sets if n_sets > 1 else 2000          # config 4: ten passes over its 64 epochs
+                    run(max(3, n_sets))
+                    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    l0 = ctx.launch_count()
+                    e0.record(stream)
+                    run(K)
+                    e1.record(stream)
+                    torch.cuda.synchronize()
+                    ms = e0.elapsed_time(e1) / K
+                    out[name] = {"workload": WORKLOAD_TEXT[name], "steps": K, "us_per_step": 1e3 * ms,
+                                 "value": bytes_per_step(w) / (ms * 1e-3) / 1e9, "unit": UNIT,
+                                 "descs_per_s": descs_per_step(w) / (ms * 1e-3), "gpu_launches": int(ctx.launch_count() - l0),
+                                 "step": "one epoch: one batch + one fence" + (" (stream-ordered inside the graph, one blocking "
+                                         "fence per replay of 64)" if graph is not None else " (blocking)")}
+                    if graph is not None:
+                        graph.close()
+                finally:
+                    ctx.close()
+        except Exception as exc:       # a side measurement must never cost the line
+            out[name] = {"error": repr(exc)[:200]}
+    return out
+
+
 def run_cuda(args):
     import torch
     import paper_2509_01425_b200 as hicr
@@ -556,6 +620,10 @@ def run_cuda(args):
             except Exception as exc:
                 cross = {"error": repr(exc)[:300]}
 
+    others = None
+    if args.config == "bulk" and world == 1 and not args.no_other_configs:
+        others = other_configs_brief(hicr, torch, local)
+
     ms_max, ms_e2e_max = rank_max(ms, dist, "cuda"), rank_max(ms_e2e, dist, "cuda")
     bps, dps = bytes_per_step(w), descs_per_step(w)
     agg = shard_report([bps * K] * world, [dps * K] * world, ms_max, K)
@@ -618,6 +686,7 @@ def run_cuda(args):
                          "algorithmic_bytes_per_launch": bps, "pin_rate": pin,
                          "frac_of_pin_rate": (achieved / pin) if pin else None},
             "cross_gpu": cross,
+            "other_configs": others,
             "cpu_baseline": cpu, "cpu_baseline_parallel": cpu_par,
             "clocks": clk,
             "counters_ok": bool(sum(c[0] for c in counters) == sum(c[1] for c in counters)),
@@ -876,6 +945,8 @@ def main(argv=None):
     ap.add_argument("--tokens", type=int, default=None, help="channel configs: tokens per producer (default: full size)")
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-other-configs", action="store_true",
+                    help="default run: leave out the side measurements of configs 1 and 4 (`other_configs`)")
     ap.add_argument("--cpu-seconds", type=float, default=10.0, help="CPU work of the cpu_baseline leg")
     ap.add_argument("--reference-seconds", type=float, default=90.0,
                     help="--impl reference: CPU work of the whole run (each step a bounded sample)")
