@@ -150,11 +150,58 @@ struct PipeArgs {
 };
 
 // The other end's counter as this CTA knows it: the minimum of what the other end's CTAs have written here.
+// HICR_MIRROR_ACQUIRE selects how a worker orders the bulk copies (async proxy) that follow a wait behind its
+// observation of the other end's frontier (words written with st.relaxed.cluster after the writer's fence):
+//   0  plain volatile polls, nothing at the exit of the wait
+//   1  every poll is an ld.acquire.cluster; fence.proxy.async at the exit
+//   2  volatile polls; fence.acq_rel.cluster + fence.proxy.async at the exit
+//   3  volatile polls; fence.proxy.async at the exit
+//   5  volatile polls; at the exit the words are read once more with ld.acquire.cluster, then fence.proxy.async
+//   6  as 5 without the proxy fence  (DEFAULT)
+// Why 6: the ring bytes are written (bulk store) and read (bulk load) through the async proxy on both sides, so
+// no location is touched through two proxies; what the reader needs is the acquire that pairs with the writer's
+// fence + relaxed store, once per wait.  Measured on B200 (profiles/r03_mirror_acquire.md), config 5a / 5b:
+// 0: 63.5 / 4.22 ms, 6: 66.2 / 4.27, 3: 79.1 / 5.01, 5: 81.2 / 5.05, 1: 79.9 / 5.00, 2: 92.8 / 5.95 -- the proxy
+// fence at every wait exit is what costs 18-25 %, the acquire 1-4 %.
+#ifndef HICR_MIRROR_ACQUIRE
+#define HICR_MIRROR_ACQUIRE 6
+#endif
+__device__ __forceinline__ unsigned long long mirror_word_acquire(const unsigned long long *p)
+{
+    unsigned long long v;
+    asm volatile("ld.acquire.cluster.shared::cta.u64 %0, [%1];" : "=l"(v) : "r"(smem_u32(p)) : "memory");
+    return v;
+}
+__device__ __forceinline__ unsigned long long mirror_word(const unsigned long long *p)
+{
+#if HICR_MIRROR_ACQUIRE == 1
+    return mirror_word_acquire(p);
+#else
+    return *reinterpret_cast<const volatile unsigned long long *>(p);
+#endif
+}
 __device__ __forceinline__ unsigned long long mirror_min(const unsigned long long *mirror, unsigned E)
 {
-    unsigned long long v = *reinterpret_cast<const volatile unsigned long long *>(mirror);
-    for (unsigned t = 1; t < E; t++) v = min(v, *reinterpret_cast<const volatile unsigned long long *>(mirror + t));
+    unsigned long long v = mirror_word(mirror);
+    for (unsigned t = 1; t < E; t++) v = min(v, mirror_word(mirror + t));
     return v;
+}
+// At the exit of a successful wait: returns the frontier to go on with (`seen`, or what the acquire reads saw).
+__device__ __forceinline__ unsigned long long mirror_wait_done(const unsigned long long *mirror, unsigned E, unsigned long long seen)
+{
+#if HICR_MIRROR_ACQUIRE == 2
+    asm volatile("fence.acq_rel.cluster;" ::: "memory");
+#endif
+#if HICR_MIRROR_ACQUIRE == 5 || HICR_MIRROR_ACQUIRE == 6
+    seen = mirror_word_acquire(mirror);
+    for (unsigned t = 1; t < E; t++) seen = min(seen, mirror_word_acquire(mirror + t));
+#endif
+#if HICR_MIRROR_ACQUIRE == 1 || HICR_MIRROR_ACQUIRE == 2 || HICR_MIRROR_ACQUIRE == 3 || HICR_MIRROR_ACQUIRE == 5
+    fence_proxy_async();
+#endif
+    (void)mirror;
+    (void)E;
+    return seen;
 }
 
 // CL: the two ends of a ring are the two CTAs of a thread-block cluster and tell each other head / tail
@@ -262,8 +309,11 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
             }
             // room: every position of the piece has been popped ("as long as the buffer has not filled up")
             const unsigned long long end_abs = cur.a + cur.len;
-            while (tail_seen + C < end_abs)
-                tail_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->tail);
+            if (tail_seen + C < end_abs) {
+                do tail_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->tail);
+                while (tail_seen + C < end_abs);
+                if (CL) tail_seen = mirror_wait_done(mirror, E, tail_seen);
+            }
             mbar_wait(bar + s, (k / kPipeStages) & 1);
             bulk_s2g(r.ring + (cur.a % C) * T, stage + (size_t)s * a.stage_bytes, (unsigned)(cur.len * T));
             bulk_commit();
@@ -288,8 +338,11 @@ __device__ __forceinline__ void pipe_body(const PipeArgs &a, unsigned char *dyn_
     while (have) {
         const unsigned s = k % kPipeStages;
         const unsigned long long end_abs = cur.a + cur.len;
-        while (head_seen < end_abs)
-            head_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->head);
+        if (head_seen < end_abs) {
+            do head_seen = CL ? mirror_min(mirror, E) : ld_acquire(&st->head);
+            while (head_seen < end_abs);
+            if (CL) head_seen = mirror_wait_done(mirror, E, head_seen);
+        }
         if (k >= kPipeStages) bulk_wait_read<kPipeStages - 1>();   // the sink store that last read this stage
         const unsigned bytes = (unsigned)(cur.len * T);
         mbar_expect_tx(bar + s, bytes);
