@@ -75,3 +75,26 @@ def test_fails_loudly_without_a_gpu():
     # NULL arguments are rejected before any device work
     assert hicr.lib.hicr_fence(None) == hicr.HICR_ERR_INVALID_ARG
     assert hicr.lib.hicr_memcpy_batch(None, None, 0, 0, None) == hicr.HICR_ERR_INVALID_ARG
+
+
+def test_noalloc_entry_point_refuses_on_the_host_what_it_can():
+    """hicr_memcpy_batch_noalloc checks its limits and its pointers before it touches CUDA, so a
+    caller learns about a batch that cannot fit the fixed scratch array without a device, and the
+    binding's limits are the header's."""
+    import paper_2509_01425_b200 as hicr
+    text = open(HEADER).read()
+    for name in ("HICR_NOALLOC_MAX_DESCS", "HICR_NOALLOC_MAX_SLOTS", "HICR_NOALLOC_MAX_CHUNKS"):
+        assert int(re.search(r"#define\s+%s\s+(\d+)u" % name, text).group(1)) == getattr(hicr, name), name
+    body = re.search(r"typedef struct hicr_raw_slot \{(.*?)\} hicr_raw_slot_t;", text, flags=re.S).group(1)
+    assert re.findall(r"(\w+);", body) == list(hicr.RAW_SLOT_DTYPE.names) and hicr.RAW_SLOT_DTYPE.itemsize == 16
+    call = hicr.lib.hicr_memcpy_batch_noalloc
+    p = 0x1000          # never dereferenced: every case below is refused first
+    assert call(0, None, p, 2, p, hicr.HICR_NOALLOC_MAX_DESCS + 1, p, p) == hicr.HICR_ERR_NO_CAPACITY
+    assert call(0, None, p, hicr.HICR_NOALLOC_MAX_SLOTS + 1, p, 1, p, p) == hicr.HICR_ERR_NO_CAPACITY
+    assert call(0, None, p, 2, p, 1, p, None) == hicr.HICR_ERR_INVALID_ARG      # no result words
+    assert call(0, None, None, 2, p, 1, p, p) == hicr.HICR_ERR_INVALID_ARG      # slots promised, none given
+    assert call(0, None, p, 2, None, 1, p, p) == hicr.HICR_ERR_INVALID_ARG      # descriptors promised, none given
+    assert call(-1, None, p, 2, p, 1, p, p) == hicr.HICR_ERR_INVALID_ARG
+    with pytest.raises(hicr.HicrError) as e:
+        hicr.memcpy_batch_noalloc(0, 0, p, 2, p, hicr.HICR_NOALLOC_MAX_DESCS + 1, p, p)
+    assert e.value.status == hicr.HICR_ERR_NO_CAPACITY
